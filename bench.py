@@ -1,0 +1,303 @@
+#!/usr/bin/env python
+"""Benchmark of the nuclear-pasta MD hot path (BASELINE.json metric: MD steps/s and pair interactions/s
+at 409 600 nucleons; fraction of the B200 FP32/SFU roofline).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config 4|2]
+
+One "step" = one full MD step (first half kick + drift + box scaling + wrap, cell-list build, pair
+force + energy, second half kick + KE + thermostat) of BASELINE config 4 (409 600 nucleons, Y_P = 0.30,
+n = 0.08 fm^-3, T = 0.5 MeV, r_c = 20 fm, rescale every 10 steps) on seeded synthetic input.  The path
+does not shard ("replicas only"), so --gpus N runs N independent replicas, one process
+per GPU, and reports their aggregate.  Prints ONE JSON line on rank 0.
+"""
+import argparse
+import json
+import math
+import os
+import statistics
+import subprocess
+import sys
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+from paper_1412_8502_b200 import inputs  # noqa: E402
+
+SM_COUNT = 148
+FP32_LANES_PER_SM = 128  # 4 SMSPs x 32 lanes, one warp instruction per SMSP per clock
+MUFU_LANES_PER_SM = 16
+
+
+def peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    sm_max_mhz, hbm, src = 1965.0, 6650.0, "fallback (B200_PROFILING.md)"
+    if os.path.exists(path):
+        try:
+            m = json.load(open(path))
+            sm_max_mhz, hbm, src = float(m.get("sm_max_mhz", sm_max_mhz)), float(m.get("hbm_gbs", hbm)), "MEASURED_PEAKS.json"
+        except Exception:
+            pass
+    return sm_max_mhz, hbm, src
+
+
+def algorithmic_cost(Y_P):
+    """FP32 lane-instructions and MUFU ops per ordered in-range pair:
+    17 + 1 for a nuclear-only pair, +8 and +2 for a proton-proton pair (fraction Y_P^2 when uniform)."""
+    fpp = Y_P * Y_P
+    return 17.0 + 8.0 * fpp, 1.0 + 2.0 * fpp
+
+
+class ClockSampler:
+    """nvidia-smi clocks + throttle reasons sampled during the timed region (B200_PROFILING.md)."""
+
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.proc = None
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(index), "--query-gpu=" + self.Q,
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+        except Exception:
+            self.proc = None
+
+    def stop(self):
+        out = {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
+        if self.proc is None:
+            return out
+        time.sleep(0.15)
+        self.proc.terminate()
+        try:
+            text = self.proc.communicate(timeout=5)[0]
+        except Exception:
+            self.proc.kill()
+            text = ""
+        sm, mx, reasons = [], [], set()
+        names = ("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap")
+        for line in text.splitlines():
+            f = [t.strip() for t in line.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                sm.append(float(f[0]))
+                mx.append(float(f[1]))
+            except ValueError:
+                continue
+            for name, val in zip(names, f[3:7]):
+                if val.lower().startswith("active"):
+                    reasons.add(name)
+        if sm:
+            out.update(sm_mhz=statistics.median(sm), sm_max_mhz=max(mx), reasons=sorted(reasons), samples=len(sm))
+        return out
+
+
+def cpu_baseline(cfg, budget_s, seed=1):
+    """The oracle as it stands, timed on the host cores on a bounded sample: forces + energies of n_sample
+    targets against ALL N sources (the all-pairs definition), scaled by N / n_sample to one force
+    evaluation = one MD step (the O(N) integrator update is not in the sample; the force
+    calculation is "by far the most time consuming part of each time step")."""
+    import numpy as np
+
+    import oracle
+
+    c = inputs.CONFIGS[cfg]
+    x, v, is_p, L = inputs.config_state(cfg, seed)
+    p = oracle.Params(r_c=c["r_c"])
+    cores = oracle.num_threads()
+    rng = np.random.default_rng(0)
+    probe = np.sort(rng.choice(c["N"], size=4 * cores, replace=False))
+    t0 = time.perf_counter()
+    oracle.forces(x, is_p, L, p, targets=probe)
+    per_target = (time.perf_counter() - t0) / len(probe)
+    n_sample = int(max(cores, min(c["N"], budget_s / max(per_target, 1e-9))))
+    n_sample -= n_sample % cores
+    sample = np.sort(rng.choice(c["N"], size=n_sample, replace=False))
+    t0 = time.perf_counter()
+    _, _, _, diag = oracle.forces(x, is_p, L, p, targets=sample)
+    dt = time.perf_counter() - t0
+    step_s = dt * c["N"] / n_sample
+    return {
+        "value": 1.0 / step_s, "unit": "steps/s", "cores": cores, "kind": "oracle",
+        "sample": "FP64 all-pairs forces+energy of %d of %d targets vs all %d sources in %.1f s, scaled by N/n_sample"
+                  % (n_sample, c["N"], c["N"], dt),
+        "ordered_pairs_per_s": diag["ordered_pairs"] / dt,
+    }
+
+
+def run_reference(args, rank, world):
+    """--impl reference: the oracle on the host cores, same metric/config; each step a bounded sample."""
+    if rank != 0:
+        return
+    c = inputs.CONFIGS[args.config]
+    total = max(1, args.steps + args.warmup)
+    per_step = min(8.0, 150.0 / total)
+    vals = []
+    base = None
+    for k in range(total):
+        base = cpu_baseline(args.config, per_step, seed=1)
+        if k >= args.warmup:
+            vals.append(base["value"])
+    v = len(vals) / sum(1.0 / a for a in vals)
+    line = {
+        "impl": "reference", "metric": "md_steps_per_s", "value": v, "unit": "steps/s", "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 / v, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": workload_config(args.config, world),
+        "cpu_baseline": {"value": v, "unit": "steps/s", "cores": base["cores"], "kind": "oracle", "sample": base["sample"]},
+        "e2e": {"value": v, "unit": "steps/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+    }
+    print(json.dumps(line), flush=True)
+
+
+def workload_config(cfg, world):
+    c = inputs.CONFIGS[cfg]
+    return {
+        "workload": "BASELINE config %d: %d nucleons, Y_P=%.2f, n=%.3f fm^-3, T=%.2f MeV, r_c=%g fm, dt=%g fm/c, "
+                    "velocity rescale every %d steps, seeded uniform-random start" % (
+                        cfg, c["N"], c["Y_P"], c["density"], c["T"], c["r_c"], c["dt"], c["thermostat_interval"]),
+        "N": c["N"], "parallelism": "replicas x%d (one GPU each, no data-path collective)" % world,
+        "l2": "flushed between timed steps (256 MB write); the 50 MB MD state is otherwise L2-resident by nature",
+    }
+
+
+def run_ours(args, rank, world, local_rank):
+    import torch
+
+    import paper_1412_8502_b200 as pasta
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the product path has no CPU fallback")
+    torch.cuda.set_device(local_rank)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+    c = inputs.CONFIGS[args.config]
+    N = c["N"]
+    prm = pasta.default_params(r_c=c["r_c"], thermostat_interval=c["thermostat_interval"],
+                               scale_per_step=c["scale_per_step"])
+    if args.variant is not None:
+        prm.force_variant = args.variant
+    if args.subdiv is not None:
+        prm.cell_subdiv = args.subdiv
+    sim = pasta.Sim(N, c["Y_P"], c["density"], c["T"], params=prm, seed=1 + rank)
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    # ---- device-resident timing: K single steps, each bracketed by events, L2 flushed in between ----
+    for _ in range(max(args.warmup, 3)):
+        sim.step(1, c["dt"])
+    torch.cuda.synchronize()
+    sim.set_timing(True)
+    n0 = sim.launch_count()
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    barrier()
+    sampler = ClockSampler(local_rank) if rank == 0 else None
+    t_wall0 = time.perf_counter()
+    for a, b in ev:
+        flush.zero_()
+        a.record()
+        sim.step(1, c["dt"])
+        b.record()
+    barrier()
+    t_wall = time.perf_counter() - t_wall0
+    clocks = sampler.stop() if sampler else None
+    launches = sim.launch_count() - n0
+    tm = sim.get_timing()
+    sim.set_timing(False)
+    dev_s = sum(a.elapsed_time(b) for a, b in ev) * 1e-3
+    pairs = sim.pair_count()  # ordered in-range pairs of the current configuration
+    ke, pe = sim.energy()
+
+    # ---- end to end through the C ABI with HOST buffers: every step copies the state in and out ----
+    hx, hv, hF = (torch.empty((N, 3), dtype=torch.float64).pin_memory() for _ in range(3))
+    L, _ = sim.get_state_host(hx, hv, hF)
+    e2e_steps = max(3, min(args.steps, 50))
+    for _ in range(2):
+        sim.set_state_host(hx, hv, None, hF, L)
+        sim.step(1, c["dt"])
+        L, _ = sim.get_state_host(hx, hv, hF)
+    barrier()
+    t0 = time.perf_counter()
+    for _ in range(e2e_steps):
+        sim.set_state_host(hx, hv, None, hF, L)
+        sim.step(1, c["dt"])
+        L, _ = sim.get_state_host(hx, hv, hF)
+    barrier()
+    e2e_s = time.perf_counter() - t0
+
+    t = torch.tensor([dev_s, e2e_s], dtype=torch.float64, device="cuda")
+    if dist is not None:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    dev_s, e2e_s = t.tolist()
+    if rank == 0:
+        sm_max_mhz, hbm_gbs, peak_src = peaks()
+        c_fp32, c_mufu = algorithmic_cost(c["Y_P"])
+        k2_s = tm["force_ms"] * 1e-3 / max(1, tm["force_evals"])
+        fp32_peak = SM_COUNT * FP32_LANES_PER_SM * sm_max_mhz * 1e6
+        mufu_peak = SM_COUNT * MUFU_LANES_PER_SM * sm_max_mhz * 1e6
+        achieved = pairs * c_fp32 / k2_s
+        roof_pairs = min(fp32_peak / c_fp32, mufu_peak / c_mufu)
+        steps_per_s = world * args.steps / dev_s
+        line = {
+            "metric": "md_steps_per_s", "value": steps_per_s, "unit": "steps/s", "n_gpus": world,
+            "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": 1e3 * dev_s / args.steps,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+            "config": workload_config(args.config, world),
+            "pair_interactions_per_s": {"unordered": 0.5 * pairs * steps_per_s, "ordered": pairs * steps_per_s,
+                                        "ordered_pairs_per_step": pairs},
+            "kernel_ms": {"cells": tm["cells_ms"] / max(1, tm["force_evals"]), "pair_force": 1e3 * k2_s,
+                          "integrate": tm["integrate_ms"] / max(1, tm["force_evals"])},
+            "roofline": {
+                "bound": "alu", "kernel": "pair force (K2)", "achieved": achieved / 1e9, "peak": fp32_peak / 1e9,
+                "unit": "G FP32 lane-instr/s (algorithmic: %.2f per ordered in-range pair)" % c_fp32,
+                "frac": achieved / fp32_peak, "frac_of_pair_roofline": (pairs / k2_s) / roof_pairs,
+                "ordered_pairs_per_s": pairs / k2_s, "mufu_frac": (pairs * c_mufu / k2_s) / mufu_peak,
+                "peak_source": "%d SMs x %d FP32 lanes x %.0f MHz (sm_max_mhz from %s)" % (
+                    SM_COUNT, FP32_LANES_PER_SM, sm_max_mhz, peak_src),
+                "traffic": None,
+            },
+            "e2e": {"value": world * e2e_steps / e2e_s, "unit": "steps/s", "h2d_bytes_per_step": 72 * N,
+                    "d2h_bytes_per_step": 72 * N, "steps": e2e_steps,
+                    "what": "pasta_set_state_host(x,v,F) + pasta_step(1) + pasta_get_state_host(x,v,F), pinned host buffers"},
+            "gpu_launches": launches, "wall_s": t_wall, "clocks": clocks,
+            "energies_MeV": {"KE": ke, "PE": pe},
+        }
+        if not args.no_cpu_baseline and world == 1:
+            line["cpu_baseline"] = cpu_baseline(args.config, args.cpu_budget)
+        print(json.dumps(line), flush=True)
+    sim.close()
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=100)
+    ap.add_argument("--warmup", type=int, default=10)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", type=int, default=4, choices=[2, 4])
+    ap.add_argument("--variant", type=int, default=None, help="pasta_params.force_variant override")
+    ap.add_argument("--subdiv", type=int, default=None, help="pasta_params.cell_subdiv override")
+    ap.add_argument("--cpu-budget", type=float, default=15.0, help="seconds of oracle time for cpu_baseline")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    if args.impl == "reference":
+        run_reference(args, rank, world)
+    else:
+        run_ours(args, rank, world, local_rank)
+
+
+if __name__ == "__main__":
+    main()

@@ -1,0 +1,177 @@
+/*
+ * pasta.h -- C ABI of the B200 (sm_100a) nuclear-pasta molecular-dynamics hot path.
+ *
+ * The library computes, entirely in hand-written CUDA kernels on ONE GPU, the per-step two-body
+ * force/energy evaluation, the counting-sort cell list that feeds it, the fused velocity-Verlet /
+ * isokinetic-rescale / uniform box-scaling update around it, and the friends-of-friends cluster
+ * labelling of the final configuration, of the semiclassical model of Caplan, Schneider, Horowitz
+ * & Berry, "Pasta Nucleosynthesis", arXiv:1412.8502.  Citations below are "PAPER.md:<line>" (the
+ * text of the paper) and "D<n>" (a reading of an ambiguous point, listed in DESIGN.md).
+ *
+ * Conventions
+ *  - Units: lengths fm, times fm/c, energies and temperature MeV, velocities c, forces MeV/fm.
+ *  - Every function returns 0 (PASTA_OK) or a negative pasta_status; no exception crosses the ABI;
+ *    the text of the last error on the calling thread is pasta_last_error().
+ *  - "_dev" pointers are device pointers on the simulation's device, "_host" pointers are host
+ *    pointers.  The CALLER owns every buffer it passes; the library keeps no reference to them
+ *    after the call returns.  Internal buffers come from pasta_env.alloc (the Python binding hands
+ *    out torch CUDA tensors) or, if alloc is NULL, from cudaMalloc.
+ *  - All work is enqueued on pasta_env.stream and is stream-ordered.  A call that writes a scalar to
+ *    a "_host" pointer synchronises that stream before it returns; all other calls are asynchronous.
+ *  - Arrays are row-major: x, v, F are [N][3] doubles; is_proton is [N] bytes (1 = proton).
+ *  - There is no CPU fallback: without a usable CUDA device pasta_create fails with PASTA_ECUDA.
+ */
+#ifndef PASTA_H_
+#define PASTA_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum pasta_status {
+  PASTA_OK = 0,
+  PASTA_EINVAL = -1, /* bad argument (see each function) */
+  PASTA_ECUDA = -2,  /* CUDA runtime / launch failure; text in pasta_last_error() */
+  PASTA_ENOMEM = -3, /* pasta_env.alloc / cudaMalloc returned NULL */
+  PASTA_ESTATE = -4  /* call order violated (e.g. pasta_cluster_sizes before pasta_clusters) */
+} pasta_status;
+
+/*
+ * Model and algorithm parameters (POD, versioned by struct_size = sizeof(pasta_params)).
+ * pasta_params_default() fills the paper's values.
+ */
+typedef struct pasta_params {
+  uint32_t struct_size;
+  uint32_t reserved0;
+  double a, b, c, Lambda;      /* Table I: 110, -26, 24 MeV; 1.25 fm^2 (Eq. 1a-c, :75-82) */
+  double alpha_hbarc;          /* alpha*hbar*c = 1.44 MeV fm of the screened Coulomb term (Eq. 1c, :81; D4) */
+  double lambda;               /* screening length, fixed to 10 fm (D5) */
+  double r_c;                  /* single cut-off for every term of Eq. 1: a pair interacts iff r < r_c (D1, D2) */
+  double mass;                 /* nucleon mass M = 939 MeV */
+  double scale_per_step;       /* s: each pasta_step multiplies L and x by s in the drift (D9, D10); 1 = fixed box */
+  int32_t thermostat_interval; /* rescale |v| so that KE = 3/2 N T after every k-th step (D7, D8); 0 = off */
+  int32_t cell_subdiv;         /* k >= 1: cells per side = max(1, floor(L k / r_c)), width L/ncell >= r_c/k (D14) */
+  int32_t force_variant;       /* 0 = library default; >0 selects a specific pair-force kernel */
+  int32_t energy_every_step;   /* 1 (default): pasta_step evaluates per-particle energies with the forces */
+} pasta_params;
+
+/* Device environment: where internal memory and the stream come from. */
+typedef void* (*pasta_alloc_fn)(size_t bytes, void* user); /* returns a device pointer (256-B aligned) or NULL */
+typedef void (*pasta_free_fn)(void* dev_ptr, void* user);
+typedef struct pasta_env {
+  uint32_t struct_size; /* sizeof(pasta_env) */
+  int32_t device;       /* CUDA device ordinal */
+  void* stream;         /* cudaStream_t; NULL = the legacy default stream */
+  pasta_alloc_fn alloc; /* NULL = cudaMalloc/cudaFree */
+  pasta_free_fn free;
+  void* user;
+} pasta_env;
+
+typedef struct pasta_sim pasta_sim; /* opaque */
+
+/* Fill *p with the paper's constants, r_c = 20 fm, fixed box, thermostat off, library-default cell_subdiv. */
+int pasta_params_default(pasta_params* p);
+
+/*
+ * Create a simulation of N nucleons, N_p = floor(Y_P N + 1/2) protons at indices [0, N_p) (D12), in a
+ * periodic cube of side L = (N/density)^(1/3).  Initial state, generated on the device
+ * from `seed` by a counter-based generator: positions uniform in [0,L)^3, velocity components normal
+ * with variance T/M (D15).  T is also the thermostat target.  env may be NULL (device 0,
+ * default stream, cudaMalloc).
+ * EINVAL: out/p NULL, wrong struct_size, N <= 0 or N > 2^30, Y_P outside [0,1], density <= 0, T < 0,
+ * r_c <= 0, r_c > L/2 (the nearest image would be ambiguous; D3), Lambda/lambda/mass <= 0,
+ * scale_per_step <= 0, thermostat_interval < 0, cell_subdiv < 1.
+ */
+int pasta_create(pasta_sim** out, int64_t N, double Y_P, double density, double T, const pasta_params* p,
+                 uint64_t seed, const pasta_env* env);
+int pasta_destroy(pasta_sim* sim); /* frees internal buffers; NULL is a no-op */
+
+/*
+ * Force and energy of the current configuration (Eq. 1 + cut-off + nearest image):
+ *   F_i = sum_{j != i, r_ij < r_c} -(1/r) dV/dr (x_i - x_j),   PE = sum_{i<j, r_ij < r_c} V(r_ij).
+ * Rebuilds the cell list, runs the pair kernel (FP32 pair arithmetic, FP64 accumulation) and leaves
+ * the forces cached for the next pasta_step.  F_dev ([N][3], original particle order) and pe_host may
+ * each be NULL.  Synchronises the stream iff pe_host != NULL.
+ */
+int pasta_forces(pasta_sim* sim, double* F_dev, double* pe_host);
+
+/*
+ * Advance n velocity-Verlet steps of length dt (D6).  Per step:
+ *   v += (dt/2M) F;  x = s (x + dt v), L = s L, wrap into [0,L);  cell list;  F = F(x);
+ *   v += (dt/2M) F;  step count += 1;  if interval > 0 and count % interval == 0 and KE > 0:
+ *   v *= sqrt(1.5 N T / KE)   (D7, D8).
+ * Forces are evaluated first if they are stale (after create / set_state without forces / expand).
+ * Asynchronous.  EINVAL: n < 0, dt <= 0, or the box would shrink below 2 r_c.
+ */
+int pasta_step(pasta_sim* sim, int64_t n, double dt);
+
+/* One-shot uniform scaling: L *= scale, x *= scale, v unchanged, forces stale (D9).
+ * EINVAL: scale <= 0 or scale*L < 2 r_c. */
+int pasta_expand(pasta_sim* sim, double scale);
+
+/*
+ * Friends-of-friends clusters over ALL nucleons with linking length r_cl (BASELINE variant of the
+ * "MST" algorithm of; D13): connected components of {(i,j): r_ij <= r_cl}, nearest
+ * image, predicate in FP64 with a pinned operation order.  label_dev[i] (may be NULL) receives the
+ * smallest particle index of i's cluster; *n_clusters_host (may be NULL) the number of clusters.
+ * EINVAL: r_cl <= 0 or r_cl > L/2.
+ */
+int pasta_clusters(pasta_sim* sim, double r_cl, int32_t* label_dev, int64_t* n_clusters_host);
+/* After pasta_clusters: A_dev[r], Z_dev[r] = mass and charge number of the cluster labelled r, 0 elsewhere. */
+int pasta_cluster_sizes(pasta_sim* sim, int32_t* A_dev, int32_t* Z_dev);
+/* After pasta_clusters: out6_host = {free-neutron mass fraction #(A=1,Z=0)/N, number of clusters with
+ * A >= a_min, mean A, sigma A, mean Z, sigma Z over those clusters}.  Synchronises. */
+int pasta_composition(pasta_sim* sim, int32_t a_min, double* out6_host);
+
+/* State accessors.  Any pointer may be NULL (skipped).  get_* with a host scalar synchronises. */
+int pasta_get_state(pasta_sim* sim, double* x_dev, double* v_dev, uint8_t* is_proton_dev, double* L_host,
+                    int64_t* step_host);
+/* Replace the state.  x is wrapped into [0,L) on the device.  F_dev != NULL supplies the forces F(x)
+ * of that configuration (a restart); NULL marks them stale.  EINVAL: L < 2 r_c. */
+int pasta_set_state(pasta_sim* sim, const double* x_dev, const double* v_dev, const uint8_t* is_proton_dev,
+                    const double* F_dev, double L);
+/* The same with HOST buffers (pinned memory recommended): asynchronous copies on the stream, then as
+ * above.  get_state_host synchronises before returning.  F_host may be NULL. */
+int pasta_get_state_host(pasta_sim* sim, double* x_host, double* v_host, double* F_host, double* L_host,
+                         int64_t* step_host);
+int pasta_set_state_host(pasta_sim* sim, const double* x_host, const double* v_host, const uint8_t* is_proton_host,
+                         const double* F_host, double L);
+
+/*
+ * Cell assignment of the current positions on the force grid (D14):
+ *   ncell = max(1, floor(L k / r_c)); c = min(ncell-1, floor(x * (ncell/L))) per axis (FP64);
+ *   id = (cz ncell + cy) ncell + cx;  cell_start = exclusive prefix sum of the histogram of id.
+ * cell_id_dev [N], cell_start_dev [ncell^3 + 1] (size it with pasta_ncell first), either may be NULL.
+ */
+int pasta_cells(pasta_sim* sim, int32_t* cell_id_dev, int32_t* cell_start_dev, int32_t* ncell_side_host);
+int pasta_ncell(pasta_sim* sim, int32_t* ncell_side_host); /* no device work */
+
+/* KE = sum 1/2 M v^2 and PE of the current state (forces re-evaluated if stale).  Synchronises. */
+int pasta_energy(pasta_sim* sim, double* ke_host, double* pe_host);
+/* Per-particle energies e_i = 1/2 sum_j V(r_ij) of the last force evaluation, original order. */
+int pasta_particle_energies(pasta_sim* sim, double* e_dev);
+
+/* Number of ordered in-range pairs (i != j, r_ij < r_c) of the current configuration, counted by a
+ * kernel in the same FP32 arithmetic the force kernel uses: the work unit of the throughput metric. */
+int pasta_pair_count(pasta_sim* sim, int64_t* ordered_pairs_host);
+
+/*
+ * Instrumentation.  pasta_set_timing(sim, 1) brackets the cell-list, pair-force and integrate kernels
+ * of every later step with CUDA events on the stream; pasta_get_timing synchronises and returns the
+ * accumulated milliseconds {cell list, pair force, integrate} and the number of force evaluations
+ * timed, then resets them.  pasta_launch_count = kernels launched by this simulation so far.
+ */
+int pasta_set_timing(pasta_sim* sim, int32_t enable);
+int pasta_get_timing(pasta_sim* sim, double* ms3_host, int64_t* n_force_evals_host);
+int64_t pasta_launch_count(const pasta_sim* sim);
+
+const char* pasta_last_error(void);
+const char* pasta_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* PASTA_H_ */

@@ -1,0 +1,312 @@
+"""Thin Python binding of include/pasta.h: argument marshalling only.
+
+Every step of the path runs in the CUDA library; PyTorch supplies device memory (the library's
+internal buffers are torch tensors handed out through pasta_env.alloc), the stream, and the
+tensors results are returned in.  There is no CPU fallback: if the library cannot be built or
+loaded, or no CUDA device is usable, the calls raise.
+"""
+import ctypes as C
+import os
+
+from . import build as _build
+
+_lib = None
+
+
+class PastaError(RuntimeError):
+    def __init__(self, code, text):
+        super().__init__("pasta error %d: %s" % (code, text))
+        self.code = code
+
+
+class Params(C.Structure):
+    """pasta_params (include/pasta.h)."""
+
+    _fields_ = [
+        ("struct_size", C.c_uint32), ("reserved0", C.c_uint32),
+        ("a", C.c_double), ("b", C.c_double), ("c", C.c_double), ("Lambda", C.c_double),
+        ("alpha_hbarc", C.c_double), ("lambda_", C.c_double), ("r_c", C.c_double), ("mass", C.c_double),
+        ("scale_per_step", C.c_double),
+        ("thermostat_interval", C.c_int32), ("cell_subdiv", C.c_int32), ("force_variant", C.c_int32),
+        ("energy_every_step", C.c_int32),
+    ]
+
+
+_ALLOC_FN = C.CFUNCTYPE(C.c_void_p, C.c_size_t, C.c_void_p)
+_FREE_FN = C.CFUNCTYPE(None, C.c_void_p, C.c_void_p)
+
+
+class Env(C.Structure):
+    _fields_ = [("struct_size", C.c_uint32), ("device", C.c_int32), ("stream", C.c_void_p),
+                ("alloc", _ALLOC_FN), ("free", _FREE_FN), ("user", C.c_void_p)]
+
+
+# name -> (restype, argtypes); the ABI test checks that the library exports exactly these.
+SIGNATURES = {
+    "pasta_params_default": (C.c_int, [C.POINTER(Params)]),
+    "pasta_create": (C.c_int, [C.POINTER(C.c_void_p), C.c_int64, C.c_double, C.c_double, C.c_double,
+                               C.POINTER(Params), C.c_uint64, C.POINTER(Env)]),
+    "pasta_destroy": (C.c_int, [C.c_void_p]),
+    "pasta_forces": (C.c_int, [C.c_void_p, C.c_void_p, C.POINTER(C.c_double)]),
+    "pasta_step": (C.c_int, [C.c_void_p, C.c_int64, C.c_double]),
+    "pasta_expand": (C.c_int, [C.c_void_p, C.c_double]),
+    "pasta_clusters": (C.c_int, [C.c_void_p, C.c_double, C.c_void_p, C.POINTER(C.c_int64)]),
+    "pasta_cluster_sizes": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p]),
+    "pasta_composition": (C.c_int, [C.c_void_p, C.c_int32, C.POINTER(C.c_double)]),
+    "pasta_get_state": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.POINTER(C.c_double),
+                                  C.POINTER(C.c_int64)]),
+    "pasta_set_state": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_double]),
+    "pasta_get_state_host": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.POINTER(C.c_double),
+                                       C.POINTER(C.c_int64)]),
+    "pasta_set_state_host": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_double]),
+    "pasta_cells": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.POINTER(C.c_int32)]),
+    "pasta_ncell": (C.c_int, [C.c_void_p, C.POINTER(C.c_int32)]),
+    "pasta_energy": (C.c_int, [C.c_void_p, C.POINTER(C.c_double), C.POINTER(C.c_double)]),
+    "pasta_particle_energies": (C.c_int, [C.c_void_p, C.c_void_p]),
+    "pasta_pair_count": (C.c_int, [C.c_void_p, C.POINTER(C.c_int64)]),
+    "pasta_set_timing": (C.c_int, [C.c_void_p, C.c_int32]),
+    "pasta_get_timing": (C.c_int, [C.c_void_p, C.POINTER(C.c_double), C.POINTER(C.c_int64)]),
+    "pasta_launch_count": (C.c_int64, [C.c_void_p]),
+    "pasta_last_error": (C.c_char_p, []),
+    "pasta_version": (C.c_char_p, []),
+}
+
+
+def library_path():
+    return _build.LIB
+
+
+def load():
+    """Build (if stale) and load the C-ABI library; raises if that is impossible."""
+    global _lib
+    if _lib is None:
+        path = _build.build()
+        lib = C.CDLL(path)
+        for name, (res, args) in SIGNATURES.items():
+            fn = getattr(lib, name)
+            fn.restype = res
+            fn.argtypes = args
+        _lib = lib
+    return _lib
+
+
+def _check(rc):
+    if rc != 0:
+        raise PastaError(rc, load().pasta_last_error().decode())
+
+
+def default_params(**overrides):
+    p = Params()
+    _check(load().pasta_params_default(C.byref(p)))
+    for k, v in overrides.items():
+        if k == "lambda":
+            k = "lambda_"
+        if not hasattr(p, k):
+            raise AttributeError("pasta_params has no field %r" % k)
+        setattr(p, k, v)
+    return p
+
+
+class Sim:
+    """One simulation on one GPU (an opaque pasta_sim handle plus the torch tensors backing it)."""
+
+    def __init__(self, N, Y_P, density, T, params=None, seed=0, device=None, stream=None):
+        import torch
+
+        if not torch.cuda.is_available():
+            raise RuntimeError("pasta: no CUDA device is available and there is no CPU fallback")
+        self._torch = torch
+        self.lib = load()
+        self.device = torch.device("cuda", torch.cuda.current_device() if device is None else device)
+        self.params = params if params is not None else default_params()
+        self.N = int(N)
+        self._pool = {}
+        torch_dev = self.device
+
+        def _alloc(nbytes, _user):
+            try:
+                t = torch.empty(int(nbytes), dtype=torch.uint8, device=torch_dev)
+            except Exception:  # out of memory -> NULL -> PASTA_ENOMEM
+                return None
+            self._pool[t.data_ptr()] = t
+            return t.data_ptr()
+
+        def _free(ptr, _user):
+            self._pool.pop(ptr, None)
+
+        self._alloc_cb = _ALLOC_FN(_alloc)
+        self._free_cb = _FREE_FN(_free)
+        with torch.cuda.device(self.device):
+            st = torch.cuda.current_stream() if stream is None else stream
+        self.stream = st
+        self._env = Env(C.sizeof(Env), self.device.index, C.c_void_p(st.cuda_stream), self._alloc_cb, self._free_cb, None)
+        h = C.c_void_p()
+        _check(self.lib.pasta_create(C.byref(h), self.N, float(Y_P), float(density), float(T), C.byref(self.params),
+                                     int(seed), C.byref(self._env)))
+        self._h = h
+
+    # -- lifetime ------------------------------------------------------------------------------------
+    def close(self):
+        if getattr(self, "_h", None):
+            self.lib.pasta_destroy(self._h)
+            self._h = None
+            self._pool.clear()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *exc):
+        self.close()
+
+    def _empty(self, shape, dtype):
+        return self._torch.empty(shape, dtype=dtype, device=self.device)
+
+    def _dev(self, t, dtype, numel):
+        torch = self._torch
+        if t is None:
+            return None, None
+        t = torch.as_tensor(t)
+        t = t.to(device=self.device, dtype=dtype).contiguous()
+        if t.numel() != numel:
+            raise ValueError("expected %d elements, got %d" % (numel, t.numel()))
+        return t, C.c_void_p(t.data_ptr())
+
+    # -- the five calls of the north star -------------------------------------------------------------
+    def forces(self, want_pe=True):
+        """pasta_forces -> (F [N,3] float64 cuda tensor, PE float or None)."""
+        F = self._empty((self.N, 3), self._torch.float64)
+        pe = C.c_double()
+        _check(self.lib.pasta_forces(self._h, C.c_void_p(F.data_ptr()), C.byref(pe) if want_pe else None))
+        return F, (pe.value if want_pe else None)
+
+    def step(self, n, dt):
+        _check(self.lib.pasta_step(self._h, int(n), float(dt)))
+
+    def expand(self, scale):
+        _check(self.lib.pasta_expand(self._h, float(scale)))
+
+    def clusters(self, r_cl):
+        """pasta_clusters -> (label [N] int32 cuda tensor, n_clusters)."""
+        label = self._empty((self.N,), self._torch.int32)
+        n = C.c_int64()
+        _check(self.lib.pasta_clusters(self._h, float(r_cl), C.c_void_p(label.data_ptr()), C.byref(n)))
+        return label, n.value
+
+    # -- accessors --------------------------------------------------------------------------------------
+    def cluster_sizes(self):
+        A = self._empty((self.N,), self._torch.int32)
+        Z = self._empty((self.N,), self._torch.int32)
+        _check(self.lib.pasta_cluster_sizes(self._h, C.c_void_p(A.data_ptr()), C.c_void_p(Z.data_ptr())))
+        return A, Z
+
+    def composition(self, a_min=12):
+        out = (C.c_double * 6)()
+        _check(self.lib.pasta_composition(self._h, int(a_min), out))
+        return dict(zip(("free_n_fraction", "n_heavy", "mean_A", "sigma_A", "mean_Z", "sigma_Z"), list(out)))
+
+    def get_state(self):
+        """-> x [N,3], v [N,3] (float64 cuda), is_proton [N] (uint8 cuda), L, step."""
+        torch = self._torch
+        x = self._empty((self.N, 3), torch.float64)
+        v = self._empty((self.N, 3), torch.float64)
+        p = self._empty((self.N,), torch.uint8)
+        L, step = C.c_double(), C.c_int64()
+        _check(self.lib.pasta_get_state(self._h, C.c_void_p(x.data_ptr()), C.c_void_p(v.data_ptr()),
+                                        C.c_void_p(p.data_ptr()), C.byref(L), C.byref(step)))
+        return x, v, p, L.value, step.value
+
+    def set_state(self, x, v, is_proton=None, F=None, L=None):
+        torch = self._torch
+        if L is None:
+            L = self.box_length()
+        keep = []
+        ptrs = []
+        for t, dt, n in ((x, torch.float64, 3 * self.N), (v, torch.float64, 3 * self.N),
+                         (is_proton, torch.uint8, self.N), (F, torch.float64, 3 * self.N)):
+            tt, ptr = self._dev(t, dt, n)
+            keep.append(tt)
+            ptrs.append(ptr)
+        _check(self.lib.pasta_set_state(self._h, ptrs[0], ptrs[1], ptrs[2], ptrs[3], float(L)))
+        self.stream.synchronize()  # `keep` may be temporaries
+        del keep
+
+    def set_state_host(self, x, v, is_proton=None, F=None, L=None):
+        """Host (ideally pinned) torch CPU tensors -> device, asynchronously on the stream."""
+        if L is None:
+            L = self.box_length()
+
+        def hp(t):
+            return None if t is None else C.c_void_p(t.data_ptr())
+
+        _check(self.lib.pasta_set_state_host(self._h, hp(x), hp(v), hp(is_proton), hp(F), float(L)))
+
+    def get_state_host(self, x=None, v=None, F=None):
+        def hp(t):
+            return None if t is None else C.c_void_p(t.data_ptr())
+
+        L, step = C.c_double(), C.c_int64()
+        _check(self.lib.pasta_get_state_host(self._h, hp(x), hp(v), hp(F), C.byref(L), C.byref(step)))
+        return L.value, step.value
+
+    def box_length(self):
+        L = C.c_double()
+        _check(self.lib.pasta_get_state(self._h, None, None, None, C.byref(L), None))
+        return L.value
+
+    def step_count(self):
+        n = C.c_int64()
+        _check(self.lib.pasta_get_state(self._h, None, None, None, None, C.byref(n)))
+        return n.value
+
+    def ncell(self):
+        n = C.c_int32()
+        _check(self.lib.pasta_ncell(self._h, C.byref(n)))
+        return n.value
+
+    def cells(self):
+        """-> cell_id [N] int32, cell_start [ncell^3+1] int32 (cuda), ncell per side."""
+        nc = self.ncell()
+        cid = self._empty((self.N,), self._torch.int32)
+        start = self._empty((nc ** 3 + 1,), self._torch.int32)
+        n = C.c_int32()
+        _check(self.lib.pasta_cells(self._h, C.c_void_p(cid.data_ptr()), C.c_void_p(start.data_ptr()), C.byref(n)))
+        assert n.value == nc
+        return cid, start, nc
+
+    def energy(self):
+        ke, pe = C.c_double(), C.c_double()
+        _check(self.lib.pasta_energy(self._h, C.byref(ke), C.byref(pe)))
+        return ke.value, pe.value
+
+    def kinetic(self):
+        ke = C.c_double()
+        _check(self.lib.pasta_energy(self._h, C.byref(ke), None))
+        return ke.value
+
+    def particle_energies(self):
+        e = self._empty((self.N,), self._torch.float64)
+        _check(self.lib.pasta_particle_energies(self._h, C.c_void_p(e.data_ptr())))
+        return e
+
+    def pair_count(self):
+        n = C.c_int64()
+        _check(self.lib.pasta_pair_count(self._h, C.byref(n)))
+        return n.value
+
+    def set_timing(self, enable=True):
+        _check(self.lib.pasta_set_timing(self._h, 1 if enable else 0))
+
+    def get_timing(self):
+        ms = (C.c_double * 3)()
+        n = C.c_int64()
+        _check(self.lib.pasta_get_timing(self._h, ms, C.byref(n)))
+        return {"cells_ms": ms[0], "force_ms": ms[1], "integrate_ms": ms[2], "force_evals": n.value}
+
+    def launch_count(self):
+        return int(self.lib.pasta_launch_count(self._h))

@@ -1,0 +1,227 @@
+// K1 -- counting-sort cell list (cubical cells, here rebuilt
+// every step on the GPU instead of a halo'd neighbour list on the CPU).
+//
+// Layout produced (all in HBM, L2-resident at these sizes):
+//   cell_id[N]            O3 id (cz*ncell + cy)*ncell + cx of every particle, original order
+//   bin_start[2*nc3 + 1]  exclusive scan over (species, cell) bins; bin = (is_proton ? 0 : nc3) + id,
+//                         so sorted slots [0, Np) are protons and [Np, N) neutrons, each cell-sorted
+//   perm[N]               sorted slot -> original index, ascending inside a bin (deterministic order)
+//   pos4[N]  (float4)     sigma * (x - cell origin) for x, y, z  and .w = (float)cx
+//   cxyz[N]               cx | cy << 10 | cz << 20
+#include "pasta_internal.cuh"
+
+namespace pasta {
+
+Grid make_grid(double L, double r_c, int32_t k) {
+  Grid g;
+  double q = floor(L * (double)k / r_c);
+  if (q < 1.0) q = 1.0;
+  if (q > 1023.0) q = 1023.0;  // cx, cy, cz are packed in 10 bits each
+  g.ncell = (int32_t)q;
+  g.nc3 = (int64_t)g.ncell * g.ncell * g.ncell;
+  g.inv_w = (double)g.ncell / L;
+  g.w = L / (double)g.ncell;
+  return g;
+}
+
+// c = min(ncell-1, floor(x * inv_w)) -- a single correctly rounded FP64 multiply, then floor (D14).
+__device__ __forceinline__ int cell_coord(double x, double inv_w, int ncell) {
+  int q = (int)floor(__dmul_rn(x, inv_w));
+  q = q > ncell - 1 ? ncell - 1 : q;
+  return q < 0 ? 0 : q;
+}
+
+__global__ void k1_count_kernel(int64_t N, const double* __restrict__ x, const uint8_t* __restrict__ is_p,
+                                double inv_w, int ncell, int nc3, int32_t* __restrict__ cell_id,
+                                int32_t* __restrict__ bin_count) {
+  int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= N) return;
+  int cx = cell_coord(x[3 * i + 0], inv_w, ncell);
+  int cy = cell_coord(x[3 * i + 1], inv_w, ncell);
+  int cz = cell_coord(x[3 * i + 2], inv_w, ncell);
+  int id = (cz * ncell + cy) * ncell + cx;
+  cell_id[i] = id;
+  atomicAdd(&bin_count[(is_p[i] ? 0 : nc3) + id], 1);
+}
+
+// ---- exclusive scan: 2048 items per block, three small kernels ----------------------------------------
+constexpr int SCAN_T = 512, SCAN_ITEMS = 4, SCAN_TILE = SCAN_T * SCAN_ITEMS;
+
+__device__ __forceinline__ int block_exclusive_scan(int v, int* total) {
+  __shared__ int warp_sums[SCAN_T / 32];
+  const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+  int inc = v;
+#pragma unroll
+  for (int o = 1; o < 32; o <<= 1) {
+    int t = __shfl_up_sync(0xffffffffu, inc, o);
+    if (lane >= o) inc += t;
+  }
+  if (lane == 31) warp_sums[wid] = inc;
+  __syncthreads();
+  if (wid == 0) {
+    int ws = lane < SCAN_T / 32 ? warp_sums[lane] : 0;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+      int t = __shfl_up_sync(0xffffffffu, ws, o);
+      if (lane >= o) ws += t;
+    }
+    if (lane < SCAN_T / 32) warp_sums[lane] = ws;
+  }
+  __syncthreads();
+  int base = wid > 0 ? warp_sums[wid - 1] : 0;
+  *total = warp_sums[SCAN_T / 32 - 1];
+  return base + inc - v;
+}
+
+__global__ void __launch_bounds__(SCAN_T) scan_local_kernel(const int32_t* __restrict__ in, int32_t* __restrict__ out,
+                                                            int64_t n, int32_t* __restrict__ block_sums) {
+  const int64_t base = (int64_t)blockIdx.x * SCAN_TILE + (int64_t)threadIdx.x * SCAN_ITEMS;
+  int v[SCAN_ITEMS], s = 0;
+#pragma unroll
+  for (int k = 0; k < SCAN_ITEMS; ++k) {
+    v[k] = (base + k < n) ? in[base + k] : 0;
+    s += v[k];
+  }
+  int total;
+  int ex = block_exclusive_scan(s, &total);
+#pragma unroll
+  for (int k = 0; k < SCAN_ITEMS; ++k) {
+    if (base + k < n) out[base + k] = ex;
+    ex += v[k];
+  }
+  if (threadIdx.x == 0) block_sums[blockIdx.x] = total;
+}
+
+__global__ void __launch_bounds__(SCAN_T) scan_top_kernel(int32_t* __restrict__ block_sums, int nb,
+                                                          int32_t* __restrict__ out_total) {
+  __shared__ int carry_s;
+  if (threadIdx.x == 0) carry_s = 0;
+  __syncthreads();
+  for (int base = 0; base < nb; base += SCAN_T) {
+    int idx = base + threadIdx.x;
+    int v = idx < nb ? block_sums[idx] : 0;
+    int total;
+    int ex = block_exclusive_scan(v, &total);
+    int carry = carry_s;
+    if (idx < nb) block_sums[idx] = carry + ex;
+    __syncthreads();
+    if (threadIdx.x == 0) carry_s = carry + total;
+    __syncthreads();
+  }
+  if (threadIdx.x == 0) *out_total = carry_s;
+}
+
+__global__ void __launch_bounds__(SCAN_T) scan_add_kernel(int32_t* __restrict__ out, int64_t n,
+                                                          const int32_t* __restrict__ block_sums) {
+  const int add = block_sums[blockIdx.x];
+  const int64_t base = (int64_t)blockIdx.x * SCAN_TILE + (int64_t)threadIdx.x * SCAN_ITEMS;
+#pragma unroll
+  for (int k = 0; k < SCAN_ITEMS; ++k)
+    if (base + k < n) out[base + k] += add;
+}
+
+int scan_exclusive(Sim* s, const int32_t* in, int32_t* out, int64_t n) {
+  const int nb = (int)((n + SCAN_TILE - 1) / SCAN_TILE);
+  PASTA_TRY(buffer_reserve(s, &s->scan_tmp, sizeof(int32_t) * (size_t)(nb + 1)));
+  int32_t* tmp = s->scan_tmp.as<int32_t>();
+  scan_local_kernel<<<nb, SCAN_T, 0, s->stream>>>(in, out, n, tmp);
+  scan_top_kernel<<<1, SCAN_T, 0, s->stream>>>(tmp, nb, out + n);
+  scan_add_kernel<<<nb, SCAN_T, 0, s->stream>>>(out, n, tmp);
+  s->launches += 3;
+  PASTA_CUDA_OK(cudaGetLastError());
+  return PASTA_OK;
+}
+
+__global__ void k1_scatter_kernel(int64_t N, const int32_t* __restrict__ cell_id, const uint8_t* __restrict__ is_p,
+                                  int nc3, const int32_t* __restrict__ bin_start, int32_t* __restrict__ bin_count,
+                                  int32_t* __restrict__ perm) {
+  int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= N) return;
+  int bin = (is_p[i] ? 0 : nc3) + cell_id[i];
+  int old = atomicSub(&bin_count[bin], 1);  // leaves the histogram zeroed for the next build
+  perm[bin_start[bin] + old - 1] = (int32_t)i;
+}
+
+// One thread per bin: order the bin's members by original index, so the sorted order (and with it the
+// summation order of the force kernel) does not depend on the atomics' arrival order.
+__global__ void k1_order_kernel(int64_t nbins, const int32_t* __restrict__ bin_start, int32_t* __restrict__ perm) {
+  int64_t b = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (b >= nbins) return;
+  const int lo = bin_start[b], hi = bin_start[b + 1];
+  for (int p = lo + 1; p < hi; ++p) {
+    int key = perm[p], q = p - 1;
+    while (q >= lo && perm[q] > key) {
+      perm[q + 1] = perm[q];
+      --q;
+    }
+    perm[q + 1] = key;
+  }
+}
+
+__global__ void k1_gather_kernel(int64_t N, const double* __restrict__ x, const int32_t* __restrict__ cell_id,
+                                 const int32_t* __restrict__ perm, int ncell, double w, double sigma,
+                                 float4* __restrict__ pos4, int32_t* __restrict__ cxyz) {
+  int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (t >= N) return;
+  const int i = perm[t];
+  const int id = cell_id[i];
+  const int cx = id % ncell, cy = (id / ncell) % ncell, cz = id / (ncell * ncell);
+  float4 p;
+  p.x = (float)(sigma * (x[3 * i + 0] - (double)cx * w));
+  p.y = (float)(sigma * (x[3 * i + 1] - (double)cy * w));
+  p.z = (float)(sigma * (x[3 * i + 2] - (double)cz * w));
+  p.w = (float)cx;
+  pos4[t] = p;
+  cxyz[t] = cx | (cy << 10) | (cz << 20);
+}
+
+int k1_build(Sim* s) {
+  const int64_t N = s->N;
+  s->grid = make_grid(s->L, s->prm.r_c, s->prm.cell_subdiv);
+  const Grid& g = s->grid;
+  const int64_t nbins = 2 * g.nc3;
+  PASTA_TRY(buffer_reserve(s, &s->bin_count, sizeof(int32_t) * (size_t)(nbins + 1)));
+  PASTA_TRY(buffer_reserve(s, &s->bin_start, sizeof(int32_t) * (size_t)(nbins + 1)));
+  int32_t* cnt = s->bin_count.as<int32_t>();
+  int32_t* start = s->bin_start.as<int32_t>();
+  PASTA_CUDA_OK(cudaMemsetAsync(cnt, 0, sizeof(int32_t) * (size_t)(nbins + 1), s->stream));
+  const int B = 256;
+  k1_count_kernel<<<grid_for(N, B), B, 0, s->stream>>>(N, s->x.as<double>(), s->is_p.as<uint8_t>(), g.inv_w, g.ncell,
+                                                       (int)g.nc3, s->cell_id.as<int32_t>(), cnt);
+  s->launches += 1;
+  PASTA_TRY(scan_exclusive(s, cnt, start, nbins));
+  k1_scatter_kernel<<<grid_for(N, B), B, 0, s->stream>>>(N, s->cell_id.as<int32_t>(), s->is_p.as<uint8_t>(),
+                                                         (int)g.nc3, start, cnt, s->perm.as<int32_t>());
+  k1_order_kernel<<<grid_for(nbins, B), B, 0, s->stream>>>(nbins, start, s->perm.as<int32_t>());
+  const double sigma = sqrt(1.4426950408889634074 / (2.0 * s->prm.Lambda));
+  k1_gather_kernel<<<grid_for(N, B), B, 0, s->stream>>>(N, s->x.as<double>(), s->cell_id.as<int32_t>(),
+                                                        s->perm.as<int32_t>(), g.ncell, g.w, sigma,
+                                                        s->pos4.as<float4>(), s->cxyz.as<int32_t>());
+  s->launches += 3;
+  PASTA_CUDA_OK(cudaGetLastError());
+  return PASTA_OK;
+}
+
+// cell_start of the species-independent O3 histogram, for pasta_cells: start_p[c] + (start_n[c] - Np).
+__global__ void k1_cell_start_kernel(int64_t nc3, const int32_t* __restrict__ bin_start, int32_t* __restrict__ out) {
+  int64_t c = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (c > nc3) return;
+  const int np = bin_start[nc3];
+  out[c] = bin_start[c] + (bin_start[nc3 + c] - np);
+}
+
+int k1_export_cells(Sim* s, int32_t* cell_id_dev, int32_t* cell_start_dev) {
+  PASTA_TRY(k1_build(s));
+  if (cell_id_dev)
+    PASTA_CUDA_OK(cudaMemcpyAsync(cell_id_dev, s->cell_id.ptr, sizeof(int32_t) * (size_t)s->N,
+                                  cudaMemcpyDeviceToDevice, s->stream));
+  if (cell_start_dev) {
+    k1_cell_start_kernel<<<grid_for(s->grid.nc3 + 1, 256), 256, 0, s->stream>>>(s->grid.nc3, s->bin_start.as<int32_t>(),
+                                                                              cell_start_dev);
+    s->launches += 1;
+    PASTA_CUDA_OK(cudaGetLastError());
+  }
+  return PASTA_OK;
+}
+
+}  // namespace pasta

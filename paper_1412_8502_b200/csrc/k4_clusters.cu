@@ -1,0 +1,233 @@
+// K4 -- friends-of-friends cluster labelling by lock-free union-find (BASELINE
+// variant of the "MST" cluster algorithm; reading D13).
+//
+// Edges: all pairs with nearest-image r^2 <= r_cl^2, predicate in FP64 with a pinned operation order
+// (every operation individually rounded, no FMA contraction), so the edge set -- and with it the
+// canonical labels (smallest member index) -- is identical to a brute-force FP64 enumeration.
+// Candidates come from a cell grid of width >= r_cl (own + 26 neighbour cells).  Roots are always the
+// smaller index (hook larger root under smaller with atomicCAS), so after flattening label = min index.
+#include "pasta_internal.cuh"
+
+namespace pasta {
+
+__device__ __forceinline__ bool fof_linked(const double* __restrict__ x, int i, int j, double L, double invL,
+                                           double rcl2) {
+  double dx = __dsub_rn(x[3 * i + 0], x[3 * j + 0]);
+  double dy = __dsub_rn(x[3 * i + 1], x[3 * j + 1]);
+  double dz = __dsub_rn(x[3 * i + 2], x[3 * j + 2]);
+  dx = __dsub_rn(dx, __dmul_rn(L, rint(__dmul_rn(dx, invL))));
+  dy = __dsub_rn(dy, __dmul_rn(L, rint(__dmul_rn(dy, invL))));
+  dz = __dsub_rn(dz, __dmul_rn(L, rint(__dmul_rn(dz, invL))));
+  const double r2 = __dadd_rn(__dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy, dy)), __dmul_rn(dz, dz));
+  return r2 <= rcl2;
+}
+
+__device__ __forceinline__ int uf_find(int* parent, int i) {
+  int p = __ldcg(parent + i);
+  while (p != i) {
+    const int gp = __ldcg(parent + p);
+    if (gp != p) parent[i] = gp;  // path halving; racy but monotone (parents only ever decrease)
+    i = p;
+    p = gp;
+  }
+  return i;
+}
+
+__device__ __forceinline__ void uf_union(int* parent, int a, int b) {
+  while (true) {
+    a = uf_find(parent, a);
+    b = uf_find(parent, b);
+    if (a == b) return;
+    const int hi = a > b ? a : b, lo = a > b ? b : a;
+    const int old = atomicCAS(&parent[hi], hi, lo);
+    if (old == hi) return;
+    a = old;  // someone else hooked hi first; retry from its new parent
+    b = lo;
+  }
+}
+
+__global__ void k4_init_kernel(int64_t N, int32_t* __restrict__ parent, int32_t* __restrict__ A, int32_t* __restrict__ Z) {
+  int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= N) return;
+  parent[i] = (int32_t)i;
+  A[i] = 0;
+  Z[i] = 0;
+}
+
+__device__ __forceinline__ int cl_cell_coord(double x, double inv_w, int ncell) {
+  int q = (int)floor(__dmul_rn(x, inv_w));
+  q = q > ncell - 1 ? ncell - 1 : q;
+  return q < 0 ? 0 : q;
+}
+
+__global__ void k4_count_kernel(int64_t N, const double* __restrict__ x, double inv_w, int ncell,
+                                int32_t* __restrict__ cell_id, int32_t* __restrict__ count) {
+  int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= N) return;
+  const int cx = cl_cell_coord(x[3 * i + 0], inv_w, ncell), cy = cl_cell_coord(x[3 * i + 1], inv_w, ncell),
+            cz = cl_cell_coord(x[3 * i + 2], inv_w, ncell);
+  const int id = (cz * ncell + cy) * ncell + cx;
+  cell_id[i] = id;
+  atomicAdd(&count[id], 1);
+}
+
+__global__ void k4_scatter_kernel(int64_t N, const int32_t* __restrict__ cell_id, const int32_t* __restrict__ start,
+                                  int32_t* __restrict__ count, int32_t* __restrict__ perm) {
+  int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= N) return;
+  const int id = cell_id[i];
+  const int old = atomicSub(&count[id], 1);
+  perm[start[id] + old - 1] = (int32_t)i;
+}
+
+// One thread per particle i: link with every j < i in the 27 surrounding cells that satisfies the predicate.
+__global__ void k4_link_cells_kernel(int64_t N, const double* __restrict__ x, const int32_t* __restrict__ cell_id,
+                                     const int32_t* __restrict__ start, const int32_t* __restrict__ perm, int ncell,
+                                     double L, double invL, double rcl2, int32_t* __restrict__ parent) {
+  int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= N) return;
+  const int id = cell_id[i];
+  const int cx = id % ncell, cy = (id / ncell) % ncell, cz = id / (ncell * ncell);
+  for (int dz = -1; dz <= 1; ++dz)
+    for (int dy = -1; dy <= 1; ++dy)
+      for (int dx = -1; dx <= 1; ++dx) {
+        const int jx = (cx + dx + ncell) % ncell, jy = (cy + dy + ncell) % ncell, jz = (cz + dz + ncell) % ncell;
+        const int q = (jz * ncell + jy) * ncell + jx;
+        for (int s = start[q]; s < start[q + 1]; ++s) {
+          const int j = perm[s];
+          if (j < i && fof_linked(x, j, (int)i, L, invL, rcl2)) uf_union(parent, (int)i, j);
+        }
+      }
+}
+
+// Small boxes (fewer than 3 cells per side): all pairs j < i.
+__global__ void k4_link_all_kernel(int64_t N, const double* __restrict__ x, double L, double invL, double rcl2,
+                                   int32_t* __restrict__ parent) {
+  int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= N) return;
+  for (int j = 0; j < (int)i; ++j)
+    if (fof_linked(x, j, (int)i, L, invL, rcl2)) uf_union(parent, (int)i, j);
+}
+
+__global__ void k4_flatten_kernel(int64_t N, int32_t* __restrict__ parent, const uint8_t* __restrict__ is_p,
+                                  int32_t* __restrict__ label_out, int32_t* __restrict__ A, int32_t* __restrict__ Z,
+                                  unsigned long long* __restrict__ n_clusters) {
+  int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= N) return;
+  const int r = uf_find(parent, (int)i);
+  if (label_out) label_out[i] = r;
+  atomicAdd(&A[r], 1);
+  if (is_p[i]) atomicAdd(&Z[r], 1);
+  if (r == (int)i) atomicAdd(n_clusters, 1ull);
+}
+
+// After flatten every parent[i] may still be an intermediate node for readers that raced; a second pass
+// makes parent[] itself the label array so that later calls can read it directly.
+__global__ void k4_store_labels_kernel(int64_t N, int32_t* __restrict__ parent) {
+  int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= N) return;
+  int r = (int)i;
+  for (int p = __ldcg(parent + r); p != r; p = __ldcg(parent + r)) r = p;
+  parent[i] = r;  // r is a root: roots are never rewritten, so concurrent readers still terminate at r
+}
+
+int k4_clusters(Sim* s, double r_cl, int32_t* label_dev, int64_t* n_clusters_host) {
+  const int64_t N = s->N;
+  const int B = 256;
+  PASTA_TRY(buffer_reserve(s, &s->cl_parent, sizeof(int32_t) * (size_t)N));
+  PASTA_TRY(buffer_reserve(s, &s->cl_A, sizeof(int32_t) * (size_t)N));
+  PASTA_TRY(buffer_reserve(s, &s->cl_Z, sizeof(int32_t) * (size_t)N));
+  int32_t* parent = s->cl_parent.as<int32_t>();
+  unsigned long long* counter = s->counters.as<unsigned long long>() + 1;
+  PASTA_CUDA_OK(cudaMemsetAsync(counter, 0, sizeof(unsigned long long), s->stream));
+  k4_init_kernel<<<grid_for(N, B), B, 0, s->stream>>>(N, parent, s->cl_A.as<int32_t>(), s->cl_Z.as<int32_t>());
+  s->launches += 1;
+
+  // grid of width >= r_cl (a hair wider, so that a rounding of x*inv_w can never separate a linked pair
+  // by two cells); at most 400 cells per side (256 MB of histogram)
+  double q = floor(s->L / (r_cl * (1.0 + 1e-9)));
+  if (q > 400.0) q = 400.0;
+  const int ncell = (int)q;
+  const double L = s->L, invL = 1.0 / s->L, rcl2 = r_cl * r_cl;
+  if (ncell >= 3) {
+    const int64_t nc3 = (int64_t)ncell * ncell * ncell;
+    PASTA_TRY(buffer_reserve(s, &s->cl_cell_id, sizeof(int32_t) * (size_t)N));
+    PASTA_TRY(buffer_reserve(s, &s->cl_perm, sizeof(int32_t) * (size_t)N));
+    PASTA_TRY(buffer_reserve(s, &s->cl_count, sizeof(int32_t) * (size_t)(nc3 + 1)));
+    PASTA_TRY(buffer_reserve(s, &s->cl_start, sizeof(int32_t) * (size_t)(nc3 + 1)));
+    int32_t* cnt = s->cl_count.as<int32_t>();
+    int32_t* start = s->cl_start.as<int32_t>();
+    PASTA_CUDA_OK(cudaMemsetAsync(cnt, 0, sizeof(int32_t) * (size_t)(nc3 + 1), s->stream));
+    k4_count_kernel<<<grid_for(N, B), B, 0, s->stream>>>(N, s->x.as<double>(), (double)ncell / L, ncell,
+                                                         s->cl_cell_id.as<int32_t>(), cnt);
+    s->launches += 1;
+    PASTA_TRY(scan_exclusive(s, cnt, start, nc3));
+    k4_scatter_kernel<<<grid_for(N, B), B, 0, s->stream>>>(N, s->cl_cell_id.as<int32_t>(), start, cnt,
+                                                           s->cl_perm.as<int32_t>());
+    k4_link_cells_kernel<<<grid_for(N, 128), 128, 0, s->stream>>>(N, s->x.as<double>(), s->cl_cell_id.as<int32_t>(),
+                                                                  start, s->cl_perm.as<int32_t>(), ncell, L, invL, rcl2,
+                                                                  parent);
+    s->launches += 2;
+  } else {
+    k4_link_all_kernel<<<grid_for(N, 128), 128, 0, s->stream>>>(N, s->x.as<double>(), L, invL, rcl2, parent);
+    s->launches += 1;
+  }
+  k4_flatten_kernel<<<grid_for(N, B), B, 0, s->stream>>>(N, parent, s->is_p.as<uint8_t>(), label_dev,
+                                                         s->cl_A.as<int32_t>(), s->cl_Z.as<int32_t>(), counter);
+  k4_store_labels_kernel<<<grid_for(N, B), B, 0, s->stream>>>(N, parent);
+  s->launches += 2;
+  PASTA_CUDA_OK(cudaGetLastError());
+  s->clusters_valid = true;
+  if (n_clusters_host) {
+    unsigned long long h = 0;
+    PASTA_CUDA_OK(cudaMemcpyAsync(&h, counter, sizeof(h), cudaMemcpyDeviceToHost, s->stream));
+    PASTA_CUDA_OK(cudaStreamSynchronize(s->stream));
+    *n_clusters_host = (int64_t)h;
+  }
+  return PASTA_OK;
+}
+
+// Composition summary from the per-cluster (A, Z) arrays with exact integer sums:
+// counters[2..8) = { #(A=1,Z=0), #heavy, sum A, sum A^2, sum Z, sum Z^2 } over clusters with A >= a_min.
+__global__ void k4_composition_kernel(int64_t N, const int32_t* __restrict__ A, const int32_t* __restrict__ Z, int a_min,
+                                      unsigned long long* __restrict__ acc) {
+  int64_t r = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (r >= N) return;
+  const unsigned long long a = (unsigned long long)A[r], z = (unsigned long long)Z[r];
+  if (a == 1 && z == 0) atomicAdd(&acc[0], 1ull);
+  if ((int)a >= a_min && a > 0) {
+    atomicAdd(&acc[1], 1ull);
+    atomicAdd(&acc[2], a);
+    atomicAdd(&acc[3], a * a);
+    atomicAdd(&acc[4], z);
+    atomicAdd(&acc[5], z * z);
+  }
+}
+
+int k4_composition(Sim* s, int32_t a_min, double* out6_host) {
+  unsigned long long* acc = s->counters.as<unsigned long long>() + 2;
+  PASTA_CUDA_OK(cudaMemsetAsync(acc, 0, 6 * sizeof(unsigned long long), s->stream));
+  k4_composition_kernel<<<grid_for(s->N, 256), 256, 0, s->stream>>>(s->N, s->cl_A.as<int32_t>(), s->cl_Z.as<int32_t>(),
+                                                                    a_min, acc);
+  s->launches += 1;
+  PASTA_CUDA_OK(cudaGetLastError());
+  unsigned long long h[6];
+  PASTA_CUDA_OK(cudaMemcpyAsync(h, acc, sizeof(h), cudaMemcpyDeviceToHost, s->stream));
+  PASTA_CUDA_OK(cudaStreamSynchronize(s->stream));
+  const double nh = (double)h[1];
+  out6_host[0] = (double)h[0] / (double)s->N;
+  out6_host[1] = nh;
+  if (nh > 0) {
+    const double mA = (double)h[2] / nh, mZ = (double)h[4] / nh;
+    const double vA = (double)h[3] / nh - mA * mA, vZ = (double)h[5] / nh - mZ * mZ;
+    out6_host[2] = mA;
+    out6_host[3] = sqrt(vA > 0 ? vA : 0);
+    out6_host[4] = mZ;
+    out6_host[5] = sqrt(vZ > 0 ? vZ : 0);
+  } else {
+    out6_host[2] = out6_host[3] = out6_host[4] = out6_host[5] = 0.0;
+  }
+  return PASTA_OK;
+}
+
+}  // namespace pasta

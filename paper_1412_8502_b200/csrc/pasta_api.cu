@@ -1,0 +1,526 @@
+// C ABI of the pasta library (include/pasta.h): argument validation, buffer ownership and the order in
+// which the kernels of one MD step are enqueued.  No arithmetic of the method lives here except the
+// host-side bookkeeping of the box length (L_{k+1} = s L_k in FP64, reading D9).
+#include <math.h>
+#include <stdarg.h>
+#include <stdio.h>
+#include <string.h>
+
+#include <new>
+
+#include "pasta_internal.cuh"
+
+namespace pasta {
+
+static thread_local char g_error[512] = "";
+
+void set_error(const char* fmt, ...) {
+  va_list ap;
+  va_start(ap, fmt);
+  vsnprintf(g_error, sizeof(g_error), fmt, ap);
+  va_end(ap);
+}
+
+int buffer_reserve(Sim* s, Buffer* b, size_t bytes) {
+  if (bytes <= b->bytes && b->ptr) return PASTA_OK;
+  buffer_release(s, b);
+  // grow geometrically so that an expanding box does not reallocate every few steps
+  size_t want = bytes + bytes / 4 + 256;
+  void* p = nullptr;
+  if (s->env.alloc) {
+    p = s->env.alloc(want, s->env.user);
+  } else {
+    if (cudaMalloc(&p, want) != cudaSuccess) p = nullptr;
+  }
+  if (!p) {
+    set_error("device allocation of %zu bytes failed", want);
+    return PASTA_ENOMEM;
+  }
+  b->ptr = p;
+  b->bytes = want;
+  return PASTA_OK;
+}
+
+void buffer_release(Sim* s, Buffer* b) {
+  if (!b->ptr) return;
+  // pending work on the stream may still use the buffer
+  cudaStreamSynchronize(s->stream);
+  if (s->env.alloc && s->env.free)
+    s->env.free(b->ptr, s->env.user);
+  else if (!s->env.alloc)
+    cudaFree(b->ptr);
+  b->ptr = nullptr;
+  b->bytes = 0;
+}
+
+static void release_all(Sim* s) {
+  Buffer* bs[] = {&s->x, &s->v, &s->F, &s->e, &s->is_p, &s->cell_id, &s->bin_count, &s->bin_start, &s->scan_tmp,
+                  &s->perm, &s->pos4, &s->cxyz, &s->partials, &s->scalars, &s->counters, &s->cl_parent, &s->cl_A,
+                  &s->cl_Z, &s->cl_cell_id, &s->cl_count, &s->cl_start, &s->cl_perm, &s->chunk_aux};
+  for (Buffer* b : bs) buffer_release(s, b);
+}
+
+static int check_sim(const Sim* s) {
+  if (!s) {
+    set_error("pasta_sim handle is NULL");
+    return PASTA_EINVAL;
+  }
+  return PASTA_OK;
+}
+
+static int use_device(const Sim* s) {
+  PASTA_CUDA_OK(cudaSetDevice(s->env.device));
+  return PASTA_OK;
+}
+
+static void timing_collect(Sim* s) {
+  for (size_t k = 0; k < s->ev_kind.size(); ++k) {
+    float ms = 0.f;
+    cudaEventSynchronize(s->evs[2 * k + 1]);
+    if (cudaEventElapsedTime(&ms, s->evs[2 * k], s->evs[2 * k + 1]) == cudaSuccess) s->ms_acc[s->ev_kind[k]] += ms;
+  }
+  s->ev_kind.clear();
+  s->ev_used = 0;
+}
+
+// Brackets a kernel group with a fresh pair of events (drained lazily, so timing does not serialise
+// the host against the stream more often than once per 1024 groups).
+struct Timer {
+  Sim* s;
+  bool on;
+  Timer(Sim* s_, int which) : s(s_), on(s_->timing) {
+    if (!on) return;
+    if (s->ev_used >= 2048) timing_collect(s);
+    while (s->evs.size() < s->ev_used + 2) {
+      cudaEvent_t e = nullptr;
+      cudaEventCreate(&e);
+      s->evs.push_back(e);
+    }
+    s->ev_kind.push_back(which);
+    cudaEventRecord(s->evs[s->ev_used], s->stream);
+  }
+  ~Timer() {
+    if (!on) return;
+    cudaEventRecord(s->evs[s->ev_used + 1], s->stream);
+    s->ev_used += 2;
+  }
+};
+
+static int evaluate_forces(Sim* s, bool with_energy) {
+  {
+    Timer t(s, 0);
+    PASTA_TRY(k1_build(s));
+  }
+  {
+    Timer t(s, 1);
+    PASTA_TRY(k2_forces(s, with_energy));
+  }
+  if (s->timing) s->n_timed += 1;
+  s->forces_valid = true;
+  s->energies_valid = with_energy;
+  return PASTA_OK;
+}
+
+}  // namespace pasta
+
+using namespace pasta;
+
+extern "C" {
+
+const char* pasta_last_error(void) { return g_error; }
+const char* pasta_version(void) { return "pasta-b200 0.1 (sm_100a)"; }
+
+int pasta_params_default(pasta_params* p) {
+  if (!p) {
+    set_error("params pointer is NULL");
+    return PASTA_EINVAL;
+  }
+  memset(p, 0, sizeof(*p));
+  p->struct_size = (uint32_t)sizeof(pasta_params);
+  p->a = 110.0;
+  p->b = -26.0;
+  p->c = 24.0;
+  p->Lambda = 1.25;
+  p->alpha_hbarc = 1.44;
+  p->lambda = 10.0;
+  p->r_c = 20.0;
+  p->mass = 939.0;
+  p->scale_per_step = 1.0;
+  p->thermostat_interval = 0;
+  p->cell_subdiv = 4;
+  p->force_variant = 0;
+  p->energy_every_step = 1;
+  return PASTA_OK;
+}
+
+static int validate_params(const pasta_params* p, double L) {
+  if (!p || p->struct_size != sizeof(pasta_params)) {
+    set_error("pasta_params is NULL or has the wrong struct_size");
+    return PASTA_EINVAL;
+  }
+  if (!(p->r_c > 0) || !(p->Lambda > 0) || !(p->lambda > 0) || !(p->mass > 0) || !(p->scale_per_step > 0) ||
+      p->thermostat_interval < 0 || p->cell_subdiv < 1 || p->cell_subdiv > 64 || p->force_variant < 0) {
+    set_error("pasta_params: r_c, Lambda, lambda, mass, scale_per_step must be > 0, thermostat_interval >= 0, "
+              "1 <= cell_subdiv <= 64");
+    return PASTA_EINVAL;
+  }
+  if (p->r_c > 0.5 * L) {
+    set_error("r_c = %g exceeds L/2 = %g: the nearest image would be ambiguous", p->r_c, 0.5 * L);
+    return PASTA_EINVAL;
+  }
+  return PASTA_OK;
+}
+
+int pasta_create(pasta_sim** out, int64_t N, double Y_P, double density, double T, const pasta_params* p,
+                 uint64_t seed, const pasta_env* env) {
+  if (!out) {
+    set_error("out is NULL");
+    return PASTA_EINVAL;
+  }
+  *out = nullptr;
+  if (N <= 0 || N > (1ll << 30) || !(Y_P >= 0.0 && Y_P <= 1.0) || !(density > 0.0) || !(T >= 0.0)) {
+    set_error("pasta_create: need 0 < N <= 2^30, 0 <= Y_P <= 1, density > 0, T >= 0");
+    return PASTA_EINVAL;
+  }
+  const double L = cbrt((double)N / density);
+  PASTA_TRY(validate_params(p, L));
+  if (env && env->struct_size != sizeof(pasta_env)) {
+    set_error("pasta_env has the wrong struct_size");
+    return PASTA_EINVAL;
+  }
+  Sim* s = new (std::nothrow) Sim();
+  if (!s) {
+    set_error("host allocation failed");
+    return PASTA_ENOMEM;
+  }
+  s->prm = *p;
+  if (env) {
+    s->env = *env;
+  } else {
+    memset(&s->env, 0, sizeof(s->env));
+    s->env.struct_size = (uint32_t)sizeof(pasta_env);
+  }
+  s->stream = (cudaStream_t)s->env.stream;
+  s->N = N;
+  s->Np = (int64_t)floor(Y_P * (double)N + 0.5);
+  s->T = T;
+  s->L = L;
+  int rc = PASTA_OK;
+  do {
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev <= s->env.device) {
+      set_error("no usable CUDA device %d (there is no CPU fallback): %s", s->env.device,
+                cudaGetErrorString(cudaGetLastError()));
+      rc = PASTA_ECUDA;
+      break;
+    }
+    if ((rc = use_device(s)) != PASTA_OK) break;
+    const size_t n = (size_t)N;
+    if ((rc = buffer_reserve(s, &s->x, 24 * n)) || (rc = buffer_reserve(s, &s->v, 24 * n)) ||
+        (rc = buffer_reserve(s, &s->F, 24 * n)) || (rc = buffer_reserve(s, &s->e, 8 * n)) ||
+        (rc = buffer_reserve(s, &s->is_p, n)) || (rc = buffer_reserve(s, &s->cell_id, 4 * n)) ||
+        (rc = buffer_reserve(s, &s->perm, 4 * n)) || (rc = buffer_reserve(s, &s->pos4, 16 * n + 4096)) ||
+        (rc = buffer_reserve(s, &s->cxyz, 4 * n)) || (rc = buffer_reserve(s, &s->partials, 8 * 8192)) ||
+        (rc = buffer_reserve(s, &s->scalars, 8 * 16)) || (rc = buffer_reserve(s, &s->counters, 8 * 16)))
+      break;
+    if (cudaMemsetAsync(s->F.ptr, 0, 24 * n, s->stream) != cudaSuccess ||
+        cudaMemsetAsync(s->e.ptr, 0, 8 * n, s->stream) != cudaSuccess ||
+        cudaMemsetAsync(s->scalars.ptr, 0, 8 * 16, s->stream) != cudaSuccess) {
+      set_error("cudaMemsetAsync failed: %s", cudaGetErrorString(cudaGetLastError()));
+      rc = PASTA_ECUDA;
+      break;
+    }
+    if ((rc = k3_init_state(s, seed)) != PASTA_OK) break;
+  } while (0);
+  if (rc != PASTA_OK) {
+    pasta_destroy(reinterpret_cast<pasta_sim*>(s));
+    return rc;
+  }
+  *out = reinterpret_cast<pasta_sim*>(s);
+  return PASTA_OK;
+}
+
+int pasta_destroy(pasta_sim* sim) {
+  Sim* s = reinterpret_cast<Sim*>(sim);
+  if (!s) return PASTA_OK;
+  cudaSetDevice(s->env.device);
+  cudaStreamSynchronize(s->stream);
+  release_all(s);
+  for (cudaEvent_t e : s->evs)
+    if (e) cudaEventDestroy(e);
+  delete s;
+  return PASTA_OK;
+}
+
+int pasta_forces(pasta_sim* sim, double* F_dev, double* pe_host) {
+  Sim* s = reinterpret_cast<Sim*>(sim);
+  PASTA_TRY(check_sim(s));
+  PASTA_TRY(use_device(s));
+  PASTA_TRY(evaluate_forces(s, true));
+  if (F_dev)
+    PASTA_CUDA_OK(cudaMemcpyAsync(F_dev, s->F.ptr, 24 * (size_t)s->N, cudaMemcpyDeviceToDevice, s->stream));
+  if (pe_host) {
+    PASTA_TRY(k3_sum(s, s->e.as<double>(), s->N, 1));
+    PASTA_CUDA_OK(cudaMemcpyAsync(pe_host, s->scalars.as<double>() + 1, sizeof(double), cudaMemcpyDeviceToHost,
+                                  s->stream));
+    PASTA_CUDA_OK(cudaStreamSynchronize(s->stream));
+  }
+  return PASTA_OK;
+}
+
+int pasta_step(pasta_sim* sim, int64_t n, double dt) {
+  Sim* s = reinterpret_cast<Sim*>(sim);
+  PASTA_TRY(check_sim(s));
+  if (n < 0 || !(dt > 0.0)) {
+    set_error("pasta_step: need n >= 0 and dt > 0");
+    return PASTA_EINVAL;
+  }
+  PASTA_TRY(use_device(s));
+  const double sc = s->prm.scale_per_step;
+  const bool energy = s->prm.energy_every_step != 0;
+  if (n > 0 && !s->forces_valid) PASTA_TRY(evaluate_forces(s, energy));
+  for (int64_t k = 0; k < n; ++k) {
+    const double L_new = sc * s->L;
+    if (s->prm.r_c > 0.5 * L_new) {
+      set_error("pasta_step: box side %g would fall below 2 r_c", L_new);
+      return PASTA_EINVAL;
+    }
+    {
+      Timer t(s, 2);
+      PASTA_TRY(k3_kick_drift(s, dt, sc, L_new));
+    }
+    s->L = L_new;
+    s->clusters_valid = false;
+    PASTA_TRY(evaluate_forces(s, energy));
+    s->step_count += 1;
+    const bool rescale = s->prm.thermostat_interval > 0 && (s->step_count % s->prm.thermostat_interval) == 0;
+    {
+      Timer t(s, 2);
+      PASTA_TRY(k3_kick_ke(s, dt, rescale));
+    }
+  }
+  return PASTA_OK;
+}
+
+int pasta_expand(pasta_sim* sim, double scale) {
+  Sim* s = reinterpret_cast<Sim*>(sim);
+  PASTA_TRY(check_sim(s));
+  if (!(scale > 0.0) || s->prm.r_c > 0.5 * scale * s->L) {
+    set_error("pasta_expand: need scale > 0 and scale*L >= 2 r_c");
+    return PASTA_EINVAL;
+  }
+  PASTA_TRY(use_device(s));
+  const double L_new = s->L * scale;
+  PASTA_TRY(k3_wrap_scale(s, scale, L_new));
+  s->L = L_new;
+  s->forces_valid = false;
+  s->energies_valid = false;
+  s->clusters_valid = false;
+  return PASTA_OK;
+}
+
+int pasta_clusters(pasta_sim* sim, double r_cl, int32_t* label_dev, int64_t* n_clusters_host) {
+  Sim* s = reinterpret_cast<Sim*>(sim);
+  PASTA_TRY(check_sim(s));
+  if (!(r_cl > 0.0) || r_cl > 0.5 * s->L) {
+    set_error("pasta_clusters: need 0 < r_cl <= L/2");
+    return PASTA_EINVAL;
+  }
+  PASTA_TRY(use_device(s));
+  return k4_clusters(s, r_cl, label_dev, n_clusters_host);
+}
+
+int pasta_cluster_sizes(pasta_sim* sim, int32_t* A_dev, int32_t* Z_dev) {
+  Sim* s = reinterpret_cast<Sim*>(sim);
+  PASTA_TRY(check_sim(s));
+  if (!s->clusters_valid) {
+    set_error("pasta_cluster_sizes: call pasta_clusters first (positions changed since)");
+    return PASTA_ESTATE;
+  }
+  PASTA_TRY(use_device(s));
+  if (A_dev) PASTA_CUDA_OK(cudaMemcpyAsync(A_dev, s->cl_A.ptr, 4 * (size_t)s->N, cudaMemcpyDeviceToDevice, s->stream));
+  if (Z_dev) PASTA_CUDA_OK(cudaMemcpyAsync(Z_dev, s->cl_Z.ptr, 4 * (size_t)s->N, cudaMemcpyDeviceToDevice, s->stream));
+  return PASTA_OK;
+}
+
+int pasta_composition(pasta_sim* sim, int32_t a_min, double* out6_host) {
+  Sim* s = reinterpret_cast<Sim*>(sim);
+  PASTA_TRY(check_sim(s));
+  if (!out6_host) {
+    set_error("out6_host is NULL");
+    return PASTA_EINVAL;
+  }
+  if (!s->clusters_valid) {
+    set_error("pasta_composition: call pasta_clusters first (positions changed since)");
+    return PASTA_ESTATE;
+  }
+  PASTA_TRY(use_device(s));
+  return k4_composition(s, a_min, out6_host);
+}
+
+int pasta_get_state(pasta_sim* sim, double* x_dev, double* v_dev, uint8_t* is_proton_dev, double* L_host,
+                    int64_t* step_host) {
+  Sim* s = reinterpret_cast<Sim*>(sim);
+  PASTA_TRY(check_sim(s));
+  PASTA_TRY(use_device(s));
+  const size_t n = (size_t)s->N;
+  if (x_dev) PASTA_CUDA_OK(cudaMemcpyAsync(x_dev, s->x.ptr, 24 * n, cudaMemcpyDeviceToDevice, s->stream));
+  if (v_dev) PASTA_CUDA_OK(cudaMemcpyAsync(v_dev, s->v.ptr, 24 * n, cudaMemcpyDeviceToDevice, s->stream));
+  if (is_proton_dev) PASTA_CUDA_OK(cudaMemcpyAsync(is_proton_dev, s->is_p.ptr, n, cudaMemcpyDeviceToDevice, s->stream));
+  if (L_host) *L_host = s->L;
+  if (step_host) *step_host = s->step_count;
+  if (L_host || step_host) PASTA_CUDA_OK(cudaStreamSynchronize(s->stream));
+  return PASTA_OK;
+}
+
+static int after_set_state(Sim* s, bool have_is_p, bool have_F, double L) {
+  s->L = L;
+  PASTA_TRY(k3_wrap_scale(s, 1.0, L));
+  if (have_is_p) {
+    PASTA_TRY(k3_count_protons(s));  // the sorted layout needs the new proton count on the host
+  }
+  s->forces_valid = have_F;
+  s->energies_valid = false;
+  s->clusters_valid = false;
+  return PASTA_OK;
+}
+
+int pasta_set_state(pasta_sim* sim, const double* x_dev, const double* v_dev, const uint8_t* is_proton_dev,
+                    const double* F_dev, double L) {
+  Sim* s = reinterpret_cast<Sim*>(sim);
+  PASTA_TRY(check_sim(s));
+  if (!(L > 0.0) || s->prm.r_c > 0.5 * L) {
+    set_error("pasta_set_state: need L >= 2 r_c");
+    return PASTA_EINVAL;
+  }
+  PASTA_TRY(use_device(s));
+  const size_t n = (size_t)s->N;
+  if (x_dev) PASTA_CUDA_OK(cudaMemcpyAsync(s->x.ptr, x_dev, 24 * n, cudaMemcpyDeviceToDevice, s->stream));
+  if (v_dev) PASTA_CUDA_OK(cudaMemcpyAsync(s->v.ptr, v_dev, 24 * n, cudaMemcpyDeviceToDevice, s->stream));
+  if (is_proton_dev) PASTA_CUDA_OK(cudaMemcpyAsync(s->is_p.ptr, is_proton_dev, n, cudaMemcpyDeviceToDevice, s->stream));
+  if (F_dev) PASTA_CUDA_OK(cudaMemcpyAsync(s->F.ptr, F_dev, 24 * n, cudaMemcpyDeviceToDevice, s->stream));
+  return after_set_state(s, is_proton_dev != nullptr, F_dev != nullptr, L);
+}
+
+int pasta_set_state_host(pasta_sim* sim, const double* x_host, const double* v_host, const uint8_t* is_proton_host,
+                         const double* F_host, double L) {
+  Sim* s = reinterpret_cast<Sim*>(sim);
+  PASTA_TRY(check_sim(s));
+  if (!(L > 0.0) || s->prm.r_c > 0.5 * L) {
+    set_error("pasta_set_state_host: need L >= 2 r_c");
+    return PASTA_EINVAL;
+  }
+  PASTA_TRY(use_device(s));
+  const size_t n = (size_t)s->N;
+  if (x_host) PASTA_CUDA_OK(cudaMemcpyAsync(s->x.ptr, x_host, 24 * n, cudaMemcpyHostToDevice, s->stream));
+  if (v_host) PASTA_CUDA_OK(cudaMemcpyAsync(s->v.ptr, v_host, 24 * n, cudaMemcpyHostToDevice, s->stream));
+  if (is_proton_host) PASTA_CUDA_OK(cudaMemcpyAsync(s->is_p.ptr, is_proton_host, n, cudaMemcpyHostToDevice, s->stream));
+  if (F_host) PASTA_CUDA_OK(cudaMemcpyAsync(s->F.ptr, F_host, 24 * n, cudaMemcpyHostToDevice, s->stream));
+  return after_set_state(s, is_proton_host != nullptr, F_host != nullptr, L);
+}
+
+int pasta_get_state_host(pasta_sim* sim, double* x_host, double* v_host, double* F_host, double* L_host,
+                         int64_t* step_host) {
+  Sim* s = reinterpret_cast<Sim*>(sim);
+  PASTA_TRY(check_sim(s));
+  PASTA_TRY(use_device(s));
+  const size_t n = (size_t)s->N;
+  if (F_host && !s->forces_valid) PASTA_TRY(evaluate_forces(s, s->prm.energy_every_step != 0));
+  if (x_host) PASTA_CUDA_OK(cudaMemcpyAsync(x_host, s->x.ptr, 24 * n, cudaMemcpyDeviceToHost, s->stream));
+  if (v_host) PASTA_CUDA_OK(cudaMemcpyAsync(v_host, s->v.ptr, 24 * n, cudaMemcpyDeviceToHost, s->stream));
+  if (F_host) PASTA_CUDA_OK(cudaMemcpyAsync(F_host, s->F.ptr, 24 * n, cudaMemcpyDeviceToHost, s->stream));
+  if (L_host) *L_host = s->L;
+  if (step_host) *step_host = s->step_count;
+  PASTA_CUDA_OK(cudaStreamSynchronize(s->stream));
+  return PASTA_OK;
+}
+
+int pasta_ncell(pasta_sim* sim, int32_t* ncell_side_host) {
+  Sim* s = reinterpret_cast<Sim*>(sim);
+  PASTA_TRY(check_sim(s));
+  if (!ncell_side_host) {
+    set_error("ncell_side_host is NULL");
+    return PASTA_EINVAL;
+  }
+  *ncell_side_host = make_grid(s->L, s->prm.r_c, s->prm.cell_subdiv).ncell;
+  return PASTA_OK;
+}
+
+int pasta_cells(pasta_sim* sim, int32_t* cell_id_dev, int32_t* cell_start_dev, int32_t* ncell_side_host) {
+  Sim* s = reinterpret_cast<Sim*>(sim);
+  PASTA_TRY(check_sim(s));
+  PASTA_TRY(use_device(s));
+  PASTA_TRY(k1_export_cells(s, cell_id_dev, cell_start_dev));
+  if (ncell_side_host) *ncell_side_host = s->grid.ncell;
+  return PASTA_OK;
+}
+
+int pasta_energy(pasta_sim* sim, double* ke_host, double* pe_host) {
+  Sim* s = reinterpret_cast<Sim*>(sim);
+  PASTA_TRY(check_sim(s));
+  PASTA_TRY(use_device(s));
+  if (pe_host) {
+    if (!s->forces_valid || !s->energies_valid) PASTA_TRY(evaluate_forces(s, true));
+    PASTA_TRY(k3_sum(s, s->e.as<double>(), s->N, 1));
+    PASTA_CUDA_OK(cudaMemcpyAsync(pe_host, s->scalars.as<double>() + 1, sizeof(double), cudaMemcpyDeviceToHost,
+                                  s->stream));
+  }
+  if (ke_host) PASTA_TRY(k3_kinetic(s, ke_host));
+  PASTA_CUDA_OK(cudaStreamSynchronize(s->stream));
+  return PASTA_OK;
+}
+
+int pasta_particle_energies(pasta_sim* sim, double* e_dev) {
+  Sim* s = reinterpret_cast<Sim*>(sim);
+  PASTA_TRY(check_sim(s));
+  if (!e_dev) {
+    set_error("e_dev is NULL");
+    return PASTA_EINVAL;
+  }
+  PASTA_TRY(use_device(s));
+  if (!s->forces_valid || !s->energies_valid) PASTA_TRY(evaluate_forces(s, true));
+  PASTA_CUDA_OK(cudaMemcpyAsync(e_dev, s->e.ptr, 8 * (size_t)s->N, cudaMemcpyDeviceToDevice, s->stream));
+  return PASTA_OK;
+}
+
+int pasta_pair_count(pasta_sim* sim, int64_t* ordered_pairs_host) {
+  Sim* s = reinterpret_cast<Sim*>(sim);
+  PASTA_TRY(check_sim(s));
+  if (!ordered_pairs_host) {
+    set_error("ordered_pairs_host is NULL");
+    return PASTA_EINVAL;
+  }
+  PASTA_TRY(use_device(s));
+  PASTA_TRY(k1_build(s));
+  return k2_pair_count(s, ordered_pairs_host);
+}
+
+int pasta_set_timing(pasta_sim* sim, int32_t enable) {
+  Sim* s = reinterpret_cast<Sim*>(sim);
+  PASTA_TRY(check_sim(s));
+  timing_collect(s);
+  s->timing = enable != 0;
+  s->ms_acc[0] = s->ms_acc[1] = s->ms_acc[2] = 0.0;
+  s->n_timed = 0;
+  return PASTA_OK;
+}
+
+int pasta_get_timing(pasta_sim* sim, double* ms3_host, int64_t* n_force_evals_host) {
+  Sim* s = reinterpret_cast<Sim*>(sim);
+  PASTA_TRY(check_sim(s));
+  PASTA_TRY(use_device(s));
+  timing_collect(s);
+  if (ms3_host)
+    for (int k = 0; k < 3; ++k) ms3_host[k] = s->ms_acc[k];
+  if (n_force_evals_host) *n_force_evals_host = s->n_timed;
+  s->ms_acc[0] = s->ms_acc[1] = s->ms_acc[2] = 0.0;
+  s->n_timed = 0;
+  return PASTA_OK;
+}
+
+int64_t pasta_launch_count(const pasta_sim* sim) {
+  const Sim* s = reinterpret_cast<const Sim*>(sim);
+  return s ? s->launches : 0;
+}
+
+}  // extern "C"

@@ -1,0 +1,137 @@
+// Internal declarations of the pasta sm_100a library (not part of the ABI).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <string>
+#include <vector>
+
+#include "pasta.h"
+
+namespace pasta {
+
+// ---- error plumbing ------------------------------------------------------------------------------
+void set_error(const char* fmt, ...);
+#define PASTA_CUDA_OK(expr)                                                                  \
+  do {                                                                                       \
+    cudaError_t err__ = (expr);                                                              \
+    if (err__ != cudaSuccess) {                                                              \
+      ::pasta::set_error("%s failed at %s:%d: %s", #expr, __FILE__, __LINE__,                \
+                         cudaGetErrorString(err__));                                         \
+      return PASTA_ECUDA;                                                                    \
+    }                                                                                        \
+  } while (0)
+#define PASTA_TRY(expr)              \
+  do {                               \
+    int rc__ = (expr);               \
+    if (rc__ != PASTA_OK) return rc__; \
+  } while (0)
+
+// ---- device buffer owned through pasta_env ---------------------------------------------------------
+struct Sim;
+struct Buffer {
+  void* ptr = nullptr;
+  size_t bytes = 0;
+  template <class T>
+  T* as() const { return reinterpret_cast<T*>(ptr); }
+};
+int buffer_reserve(Sim* s, Buffer* b, size_t bytes);  // grow-only; contents are NOT preserved
+void buffer_release(Sim* s, Buffer* b);
+
+// ---- grid of the force cell list (host-side description, recomputed whenever L changes) ------------
+struct Grid {
+  int32_t ncell = 1;   // cells per side
+  int64_t nc3 = 1;     // ncell^3
+  double inv_w = 1.0;  // ncell / L  (FP64 division on the host, D14)
+  double w = 1.0;      // L / ncell
+};
+Grid make_grid(double L, double r_c, int32_t k);
+
+// Constants of the FP32 pair arithmetic, derived on the host in FP64 (k2_force.cu explains them).
+struct PairConsts {
+  float sigma;       // coordinate pre-scale sqrt(log2(e) / (2 Lambda))
+  float inv_sigma;   // 1 / sigma
+  float rc2s;        // (sigma r_c)^2
+  float a;           // a
+  float g2a;         // 2 a / (Lambda sigma)          (force constants carry the 1/sigma of d' -> d)
+  float B_like, B_unlike;      // b + c, b - c
+  float gB_like, gB_unlike;    // B / (Lambda sigma)
+  float kappa;       // log2(e) / (sigma lambda):  exp(-r/lambda) = exp2(-kappa r')
+  float alpha_s;     // alpha sigma:                E_c = alpha_s exp2(.) / r'
+  float alpha_s2;    // alpha sigma^2:              Coulomb part of g'
+  float inv_lam_s;   // 1 / (lambda sigma):         (1/r + 1/lambda) = sigma (1/r' + inv_lam_s)
+  float v_self;      // a + b + c : V(0) of the like-species self pair, removed analytically
+};
+PairConsts make_pair_consts(const pasta_params& p);
+
+struct Sim {
+  // configuration
+  pasta_params prm;
+  pasta_env env;
+  cudaStream_t stream = nullptr;
+  int64_t N = 0;
+  int64_t Np = 0;
+  double T = 0.0;
+  double L = 0.0;
+  int64_t step_count = 0;
+  bool forces_valid = false;
+  bool energies_valid = false;
+  bool clusters_valid = false;
+  int64_t launches = 0;
+
+  // state (device)
+  Buffer x, v, F, e, is_p;  // double[N][3] x3, double[N], uint8[N]
+
+  // cell list (device)
+  Grid grid;
+  Buffer cell_id;     // int32[N]   O3 id (species-independent)
+  Buffer bin_count;   // int32[2 nc3 + 1] scratch histogram over (species, cell) bins
+  Buffer bin_start;   // int32[2 nc3 + 1] exclusive scan; protons' bins first
+  Buffer scan_tmp;    // block sums of the scan
+  Buffer perm;        // int32[N]   sorted slot -> original index
+  Buffer pos4;        // float4[N]  sorted: sigma * cell-relative position, .w = cell x index
+  Buffer cxyz;        // int32[N]   sorted: packed cell coordinates (cx | cy<<10 | cz<<20)
+
+  // reductions
+  Buffer partials;    // double[>= 4096]
+  Buffer scalars;     // double[16] device scalars: [0] KE, [1] PE, [2] rescale factor, [3..] scratch
+  Buffer counters;    // unsigned long long[16]
+
+  // clusters
+  Buffer cl_parent, cl_A, cl_Z;  // int32[N] each
+  Buffer cl_cell_id, cl_count, cl_start, cl_perm;
+
+  // pair-force chunk tables (k2_force.cu)
+  Buffer chunk_aux;
+
+  // timing: pairs of events (start, stop) tagged with the kernel group they bracket
+  bool timing = false;
+  std::vector<cudaEvent_t> evs;
+  std::vector<int> ev_kind;
+  size_t ev_used = 0;
+  double ms_acc[3] = {0, 0, 0};
+  int64_t n_timed = 0;
+};
+
+// ---- kernel launchers (one translation unit each) ---------------------------------------------------
+// K1  k1_cells.cu
+int k1_build(Sim* s);                                  // cell ids, (species,cell) counting sort, pos4/perm
+int k1_export_cells(Sim* s, int32_t* cell_id_dev, int32_t* cell_start_dev);
+int scan_exclusive(Sim* s, const int32_t* in, int32_t* out, int64_t n);  // out[0..n] (n+1 entries)
+// K2  k2_force.cu
+int k2_forces(Sim* s, bool with_energy);               // F, e in original order
+int k2_pair_count(Sim* s, int64_t* ordered_pairs_host);
+// K3  k3_integrate.cu
+int k3_init_state(Sim* s, uint64_t seed);
+int k3_kick_drift(Sim* s, double dt, double scale, double L_new);
+int k3_kick_ke(Sim* s, double dt, bool rescale);       // second half kick + KE (+ rescale)
+int k3_wrap_scale(Sim* s, double scale, double L_new); // x = wrap(scale x)
+int k3_kinetic(Sim* s, double* ke_host);
+int k3_sum(Sim* s, const double* in, int64_t n, int slot);  // deterministic sum into scalars[slot]
+int k3_count_protons(Sim* s);                          // s->Np from is_p (synchronises)
+// K4  k4_clusters.cu
+int k4_clusters(Sim* s, double r_cl, int32_t* label_dev, int64_t* n_clusters_host);
+int k4_composition(Sim* s, int32_t a_min, double* out6_host);
+
+inline int grid_for(int64_t n, int block) { return (int)((n + block - 1) / block); }
+
+}  // namespace pasta

@@ -1,0 +1,310 @@
+"""GPU parity: the CUDA path (through the C ABI) against the FP64 oracle on the same seeded inputs.
+
+Tolerances are BASELINE.json's: force relative L2 <= 1e-5 (both gates of reading D17), total PE relative
+<= 1e-6, 20-step trajectory within 1e-4 fm; cell assignments and cluster labels bit-exact.
+"""
+import math
+
+import numpy as np
+import pytest
+
+import paper_1412_8502_b200 as pasta
+from paper_1412_8502_b200 import inputs
+
+pytestmark = pytest.mark.gpu
+
+FORCE_TOL = 1e-5
+PE_TOL = 1e-6
+TRAJ_TOL = 1e-4
+
+
+def _torch():
+    import torch
+
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    return torch
+
+
+def _np(t):
+    return t.detach().cpu().numpy()
+
+
+def _oparams(orc, p):
+    return orc.Params(a=p.a, b=p.b, c=p.c, Lambda=p.Lambda, alpha=p.alpha_hbarc, lambda_=p.lambda_, r_c=p.r_c,
+                      mass=p.mass)
+
+
+def _check_forces(F_gpu, F_orc, pe_gpu=None, pe_orc=None):
+    """D17: (i) ||dF||_2/||F||_2 over the 3N vector; (ii) per particle |dF_i| <= tol max(|F_i|, F_rms)."""
+    dF = F_gpu - F_orc
+    rel = np.linalg.norm(dF) / np.linalg.norm(F_orc)
+    assert rel <= FORCE_TOL, "force relative L2 error %.3e" % rel
+    fi = np.linalg.norm(F_orc, axis=1)
+    frms = math.sqrt((fi ** 2).mean())
+    worst = (np.linalg.norm(dF, axis=1) / np.maximum(fi, frms)).max()
+    assert worst <= FORCE_TOL, "worst per-particle force error %.3e" % worst
+    if pe_orc is not None:
+        assert abs(pe_gpu - pe_orc) <= PE_TOL * abs(pe_orc), "PE %r vs %r" % (pe_gpu, pe_orc)
+    return rel, worst
+
+
+def _sim_from_arrays(x, v, is_p, L, T=1.0, **prm):
+    N = len(x)
+    density = N / L ** 3
+    p = pasta.default_params(**prm)
+    sim = pasta.Sim(N, float(np.mean(is_p)), density, T, params=p, seed=1)
+    sim.set_state(x, v, is_p, None, L)
+    return sim
+
+
+@pytest.mark.parametrize("variant", [0, 1])
+@pytest.mark.parametrize("k", [1, 2, 4])
+def test_config1_forces_energy_cells(orc, k, variant):
+    """BASELINE config 1: 2048 nucleons, Y_P = 0.30, n = 0.05, r_c = 17 (L/r_c = 2.03: degenerate grid)."""
+    c = inputs.CONFIGS[1]
+    p = pasta.default_params(r_c=c["r_c"], cell_subdiv=k, force_variant=variant)
+    with pasta.Sim(c["N"], c["Y_P"], c["density"], c["T"], params=p, seed=7) as sim:
+        x, v, is_p, L, step = sim.get_state()
+        x, v, is_p = _np(x), _np(v), _np(is_p)
+        assert L == pytest.approx(34.4710, abs=1e-4) and step == 0 and is_p.sum() == 614 and is_p[:614].all()
+        assert (x >= 0).all() and (x < L).all()
+        F, pe = sim.forces()
+        Fo, eo, peo, d = orc.forces(x, is_p, L, _oparams(orc, p))
+        _check_forces(_np(F), Fo, pe, peo)
+        e = _np(sim.particle_energies())
+        assert np.abs(e - eo).max() <= 2e-6 * np.abs(eo).max()
+        ke, pe2 = sim.energy()
+        assert pe2 == pe and ke == pytest.approx(orc.kinetic(v, 939.0), rel=1e-13)
+        assert sim.pair_count() == pytest.approx(d["ordered_pairs"], abs=max(4, 2 * d["boundary_pairs"]))
+        # cells: bit-exact
+        cid, start, nc = sim.cells()
+        assert nc == orc.ncell(L, c["r_c"], k)
+        cid_o, start_o = orc.cells(x, L, nc)
+        assert np.array_equal(_np(cid), cid_o) and np.array_equal(_np(start), start_o)
+
+
+def test_config1_trajectory_20_steps(orc):
+    """20 velocity-Verlet steps, dt = 2 fm/c, NVE, positions within 1e-4 fm (D19: nearest image)."""
+    c = inputs.CONFIGS[1]
+    p = pasta.default_params(r_c=c["r_c"], thermostat_interval=0)
+    x, v, is_p, L = inputs.config_state(1, seed=3)
+    with _sim_from_arrays(x, v, is_p, L, T=c["T"], r_c=c["r_c"]) as sim:
+        sim.step(c["steps"], c["dt"])
+        xg, vg, _, Lg, step = sim.get_state()
+        xo, vo, Lo, cnt, Fo, peo = orc.step(x, v, is_p, L, _oparams(orc, p), c["T"], 0, 1.0, c["dt"], c["steps"])
+        assert step == 20 and cnt == 20 and Lg == Lo
+        d = _np(xg) - xo
+        d -= L * np.round(d / L)
+        err = np.linalg.norm(d, axis=1).max()
+        assert err <= TRAJ_TOL, "trajectory error %.3e fm" % err
+        assert np.abs(_np(vg) - vo).max() <= 1e-6
+        ke, pe = sim.energy()
+        assert pe == pytest.approx(peo, rel=1e-5)
+
+
+@pytest.mark.parametrize("variant", [0, 1])
+@pytest.mark.parametrize("N,density,r_c,k,Y_P", [
+    (16384, 0.08, 12.0, 4, 0.3),   # many cells per side: stencil / tiled path, several tiles + ragged tail
+    (10007, 0.05, 20.0, 3, 0.4),   # prime N, ncell = 8: ragged everything
+    (4099, 0.02, 20.0, 1, 0.05),   # few protons
+    (3000, 0.08, 11.0, 5, 1.0),    # all protons
+    (3001, 0.08, 11.0, 2, 0.0),    # all neutrons
+])
+def test_forces_mid_sizes(orc, N, density, r_c, k, Y_P, variant):
+    x, v, is_p, L = inputs.uniform_state(N, Y_P, density, 1.0, seed=N)
+    with _sim_from_arrays(x, v, is_p, L, r_c=r_c, cell_subdiv=k, force_variant=variant) as sim:
+        F, pe = sim.forces()
+        Fo, eo, peo, d = orc.forces(x, is_p, L, _oparams(orc, sim.params))
+        _check_forces(_np(F), Fo, pe, peo)
+        cid, start, nc = sim.cells()
+        cid_o, start_o = orc.cells(x, L, nc)
+        assert np.array_equal(_np(cid), cid_o) and np.array_equal(_np(start), start_o)
+
+
+@pytest.mark.parametrize("variant", [0, 1])
+def test_forces_clustered_occupancy(orc, variant):
+    """Sparse + clustered cells (late decompression): empty cells, dense blobs."""
+    N = 12000
+    x, v, is_p, L = inputs.clustered_state(N, 0.2, 0.004, 0.75, seed=12)
+    with _sim_from_arrays(x, v, is_p, L, T=0.75, force_variant=variant) as sim:
+        F, pe = sim.forces()
+        Fo, eo, peo, d = orc.forces(x, is_p, L, _oparams(orc, sim.params))
+        _check_forces(_np(F), Fo, pe, peo)
+
+
+@pytest.mark.parametrize("variant", [0, 1])
+def test_edge_cases_tiny_systems(orc, variant):
+    L = 50.0
+    p = pasta.default_params(r_c=20.0, force_variant=variant)
+    op = _oparams(orc, p)
+    cases = [
+        (np.array([[1.0, 2.0, 3.0]]), [1]),                                           # a single nucleon
+        (np.array([[1.0, 2.0, 3.0], [2.5, 2.0, 3.0]]), [1, 1]),                        # one pp pair
+        (np.array([[0.0, 0.0, 0.0], [49.5, 49.75, 0.25]]), [0, 1]),                    # across three faces
+        (np.array([[5.0, 5.0, 5.0], [5.0, 5.0, 5.0], [6.0, 5.0, 5.0]]), [1, 1, 0]),   # coincident protons (D2)
+        (np.array([[1.0, 1.0, 1.0], [30.0, 30.0, 30.0]]), [0, 0]),                     # nothing in range
+    ]
+    for x, sp in cases:
+        x = np.asarray(x, dtype=float)
+        with _sim_from_arrays(x, np.zeros_like(x), np.array(sp, dtype=np.uint8), L, r_c=20.0,
+                              force_variant=variant) as sim:
+            F, pe = sim.forces()
+            Fo, eo, peo, _ = orc.forces(x, sp, L, op)
+            assert np.allclose(_np(F), Fo, rtol=2e-5, atol=1e-7), (x, _np(F), Fo)
+            assert pe == pytest.approx(peo, rel=2e-6, abs=1e-9)
+
+
+def test_thermostat_expand_and_scaled_steps(orc):
+    """Configs 2-5 mechanics on a small system: rescale every 10 steps (D7/D8), fused
+    geometric box/position scaling (D9/D10), one-shot pasta_expand."""
+    N, T = 2000, 0.75
+    x, v, is_p, L = inputs.uniform_state(N, 0.2, 0.04, T, seed=5)
+    s = 1.0005
+    prm = dict(r_c=12.0, thermostat_interval=10, scale_per_step=s)
+    with _sim_from_arrays(x, v, is_p, L, T=T, **prm) as sim:
+        op = _oparams(orc, sim.params)
+        sim.step(7, 2.0)
+        sim.step(3, 2.0)  # the counter persists across calls: the rescale falls on the 10th step
+        assert sim.kinetic() == pytest.approx(1.5 * N * T, rel=1e-12)
+        xg, vg, _, Lg, step = sim.get_state()
+        xo, vo, Lo, cnt, Fo, _ = orc.step(x, v, is_p, L, op, T, 10, s, 2.0, 10)
+        assert step == 10 and Lg == Lo and Lg == pytest.approx(L * s ** 10, rel=1e-14)
+        d = _np(xg) - xo
+        d -= Lo * np.round(d / Lo)
+        assert np.linalg.norm(d, axis=1).max() <= TRAJ_TOL
+        assert (_np(xg) >= 0).all() and (_np(xg) < Lg).all()
+        sim.step(4, 2.0)
+        assert sim.kinetic() != pytest.approx(1.5 * N * T, rel=1e-9)
+        # one-shot expansion: every pair distance x 1.3, forces stale -> re-evaluated
+        x1, v1, _, L1, _ = sim.get_state()
+        sim.expand(1.3)
+        x2, v2, _, L2, _ = sim.get_state()
+        assert L2 == L1 * 1.3 and np.array_equal(_np(v1), _np(v2))
+        xe, Le = orc.expand(_np(x1), L1, 1.3)
+        assert Le == L2 and np.abs(_np(x2) - xe).max() < 1e-10
+        F, pe = sim.forces()
+        Fo, _, peo, _ = orc.forces(_np(x2), is_p, L2, op)
+        _check_forces(_np(F), Fo, pe, peo)
+    with pytest.raises(pasta.PastaError):
+        with _sim_from_arrays(x, v, is_p, L, r_c=12.0) as sim:
+            sim.expand(0.5)  # L/2 would fall below r_c
+
+
+def test_restart_with_forces_and_host_buffers(orc):
+    """set_state_host / get_state_host (the e2e path of bench.py): a restart that supplies F continues
+    the trajectory without re-evaluating it."""
+    torch = _torch()
+    N = 3000
+    x, v, is_p, L = inputs.uniform_state(N, 0.3, 0.05, 1.0, seed=9)
+    with _sim_from_arrays(x, v, is_p, L, r_c=15.0) as a, _sim_from_arrays(x, v, is_p, L, r_c=15.0) as b:
+        a.step(4, 2.0)
+        b.step(2, 2.0)
+        hx, hv, hF = (torch.empty((N, 3), dtype=torch.float64).pin_memory() for _ in range(3))
+        Lb, stepb = b.get_state_host(hx, hv, hF)
+        assert stepb == 2
+        n_ref = a.launch_count()
+        a.step(0, 2.0)
+        n0 = b.launch_count()
+        b.set_state_host(hx, hv, None, hF, Lb)
+        b.step(2, 2.0)
+        xa, va = a.get_state()[:2]
+        xb, vb = b.get_state()[:2]
+        assert torch.equal(xa, xb) and torch.equal(va, vb)
+        # two force evaluations, not three: same launches as two plain steps plus the wrap of set_state
+        c1 = pasta.Sim(N, 0.3, 0.05, 1.0, params=a.params, seed=1)
+        c1.step(1, 2.0)
+        m0 = c1.launch_count()
+        c1.step(2, 2.0)
+        assert b.launch_count() - n0 == c1.launch_count() - m0 + 1
+        c1.close()
+
+
+def test_device_initial_state_statistics():
+    """P15 on the device generator: uniform positions, normal velocities with variance T/M (D15)."""
+    N, T = 200000, 0.5
+    p = pasta.default_params()
+    with pasta.Sim(N, 0.3, 0.08, T, params=p, seed=123) as sim, pasta.Sim(N, 0.3, 0.08, T, params=p, seed=124) as sim2:
+        x, v, is_p, L, _ = sim.get_state()
+        x, v = _np(x), _np(v)
+        assert (x >= 0).all() and (x < L).all()
+        assert np.abs(x.mean(0) / L - 0.5).max() < 4 / math.sqrt(12 * N)
+        assert x.var() / L ** 2 == pytest.approx(1 / 12, rel=0.01)
+        assert abs(v.mean()) < 4 * math.sqrt(T / 939.0 / v.size)
+        assert v.var() == pytest.approx(T / 939.0, rel=4 * math.sqrt(2.0 / v.size))
+        assert abs(((v / v.std()) ** 4).mean() - 3.0) < 0.05  # normal kurtosis
+        assert abs(np.corrcoef(x[:-1, 0], x[1:, 0])[0, 1]) < 0.01
+        assert not np.array_equal(x, _np(sim2.get_state()[0]))
+        assert int(_np(is_p).sum()) == 60000
+
+
+@pytest.mark.parametrize("N,Y_P,density,r_cl", [(3000, 0.2, 0.004, 3.0), (60000, 0.2, 0.002, 3.0), (2048, 0.3, 0.05, 2.0),
+                                                (500, 0.3, 0.5, 1.0), (300, 0.3, 0.3, 4.0)])
+def test_clusters_labels_bit_exact(orc, N, Y_P, density, r_cl):
+    """Canonical labels (minimum member index), A, Z and the composition summary: exact."""
+    x, v, is_p, L = inputs.clustered_state(N, Y_P, density, 0.75, seed=N + 1)
+    with _sim_from_arrays(x, v, is_p, L, T=0.75, r_c=min(20.0, 0.49 * L)) as sim:
+        label, n = sim.clusters(r_cl)
+        A, Z = sim.cluster_sizes()
+        fn = orc.clusters if N <= 5000 else orc.clusters_cells
+        lo, Ao, Zo, no = fn(x, is_p, L, r_cl)
+        assert n == no
+        assert np.array_equal(_np(label), lo) and np.array_equal(_np(A), Ao) and np.array_equal(_np(Z), Zo)
+        comp, compo = sim.composition(12), orc.composition(Ao, Zo, 12)
+        for key in compo:
+            assert comp[key] == pytest.approx(compo[key], rel=1e-12, abs=1e-12)
+        sim.step(1, 2.0)
+        with pytest.raises(pasta.PastaError):
+            sim.cluster_sizes()  # positions moved: stale
+
+
+def test_clusters_hand_built_chains():
+    L = 60.0
+    x = np.array([[58.0 + 2.5 * k, 7.0, 7.0] for k in range(5)]) % L
+    with _sim_from_arrays(x, np.zeros_like(x), np.array([1, 0, 0, 1, 0], dtype=np.uint8), L) as sim:
+        label, n = sim.clusters(3.0)
+        assert n == 1 and _np(label).tolist() == [0] * 5
+        label, n = sim.clusters(2.4)
+        assert n == 5 and _np(label).tolist() == list(range(5))
+        A, Z = sim.cluster_sizes()
+        assert _np(A).tolist() == [1] * 5 and _np(Z).tolist() == [1, 0, 0, 1, 0]
+
+
+def test_forces_are_reproducible_run_to_run():
+    torch = _torch()
+    x, v, is_p, L = inputs.uniform_state(20000, 0.3, 0.08, 1.0, seed=2)
+    out = []
+    for _ in range(2):
+        with _sim_from_arrays(x, v, is_p, L) as sim:
+            sim.step(3, 2.0)
+            out.append([t.clone() for t in sim.get_state()[:2]])
+    assert torch.equal(out[0][0], out[1][0]) and torch.equal(out[0][1], out[1][1])
+
+
+@pytest.mark.parametrize("cfg", [2, 4])
+def test_full_size_sampled_targets(orc, cfg):
+    """BASELINE configs 2 and 4 at full size, in bench.py's launch configuration: forces and per-particle
+    energies of sampled targets against the oracle one by one, plus size-independent properties."""
+    c = inputs.CONFIGS[cfg]
+    p = pasta.default_params(r_c=c["r_c"], thermostat_interval=c["thermostat_interval"])
+    with pasta.Sim(c["N"], c["Y_P"], c["density"], c["T"], params=p, seed=1) as sim:
+        x, v, is_p, L, _ = sim.get_state()
+        x, is_p = _np(x), _np(is_p)
+        F, pe = sim.forces()
+        F, e = _np(F), _np(sim.particle_energies())
+        rng = np.random.default_rng(cfg)
+        t = np.sort(rng.choice(c["N"], size=96 if cfg == 4 else 256, replace=False))
+        Fo, eo, _, d = orc.forces(x, is_p, L, _oparams(orc, p), targets=t)
+        dF = F[t] - Fo
+        assert np.linalg.norm(dF) / np.linalg.norm(Fo) <= FORCE_TOL
+        frms = math.sqrt((np.linalg.norm(Fo, axis=1) ** 2).mean())
+        assert (np.linalg.norm(dF, axis=1) / np.maximum(np.linalg.norm(Fo, axis=1), frms)).max() <= FORCE_TOL
+        assert abs(e[t].sum() - eo.sum()) <= PE_TOL * abs(eo.sum()) * 3
+        assert e.sum() == pytest.approx(pe, rel=1e-12)
+        assert np.abs(F.sum(0)).max() <= 1e-6 * np.abs(F).sum()          # Newton's third law
+        pairs = sim.pair_count()
+        assert pairs / c["N"] == pytest.approx(c["density"] * 4 * math.pi / 3 * c["r_c"] ** 3, rel=0.01)  # P12
+        cid, start, nc = sim.cells()
+        cid_o, start_o = orc.cells(x, L, nc)
+        assert np.array_equal(_np(cid), cid_o) and np.array_equal(_np(start), start_o)
+        sim.step(2, c["dt"])
+        assert sim.step_count() == 2
