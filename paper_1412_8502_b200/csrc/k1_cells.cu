@@ -6,7 +6,7 @@
 //   bin_start[2*nc3 + 1]  exclusive scan over (species, cell) bins; bin = (is_proton ? 0 : nc3) + id,
 //                         so sorted slots [0, Np) are protons and [Np, N) neutrons, each cell-sorted
 //   perm[N]               sorted slot -> original index, ascending inside a bin (deterministic order)
-//   pos4[N]  (float4)     sigma * (x - cell origin) for x, y, z  and .w = (float)cx
+//   pos4[N]  (float4)     sigma * (x - cell centre) for x, y, z (|.| <= sigma w / 2)  and .w = (float)cx
 //   cxyz[N]               cx | cy << 10 | cz << 20
 #include "pasta_internal.cuh"
 
@@ -167,9 +167,9 @@ __global__ void k1_gather_kernel(int64_t N, const double* __restrict__ x, const 
   const int id = cell_id[i];
   const int cx = id % ncell, cy = (id / ncell) % ncell, cz = id / (ncell * ncell);
   float4 p;
-  p.x = (float)(sigma * (x[3 * i + 0] - (double)cx * w));
-  p.y = (float)(sigma * (x[3 * i + 1] - (double)cy * w));
-  p.z = (float)(sigma * (x[3 * i + 2] - (double)cz * w));
+  p.x = (float)(sigma * (x[3 * i + 0] - ((double)cx + 0.5) * w));
+  p.y = (float)(sigma * (x[3 * i + 1] - ((double)cy + 0.5) * w));
+  p.z = (float)(sigma * (x[3 * i + 2] - ((double)cz + 0.5) * w));
   p.w = (float)cx;
   pos4[t] = p;
   cxyz[t] = cx | (cy << 10) | (cz << 20);
