@@ -158,6 +158,11 @@ int pasta_particle_energies(pasta_sim* sim, double* e_dev);
  * kernel in the same FP32 arithmetic the force kernel uses: the work unit of the throughput metric. */
 int pasta_pair_count(pasta_sim* sim, int64_t* ordered_pairs_host);
 
+/* Work statistics of one evaluation with the chunk pair kernel: out3_host = {raw candidates streamed from
+ * the cell rows, candidates that survived the bounding-sphere test, pair evaluations executed}.
+ * Synchronises.  (ordered in-range pairs / pair evaluations = the kernel's useful-work fraction.) */
+int pasta_force_stats(pasta_sim* sim, int64_t* out3_host);
+
 /*
  * Instrumentation.  pasta_set_timing(sim, 1) brackets the cell-list, pair-force and integrate kernels
  * of every later step with CUDA events on the stream; pasta_get_timing synchronises and returns the

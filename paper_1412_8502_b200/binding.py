@@ -64,6 +64,7 @@ SIGNATURES = {
     "pasta_energy": (C.c_int, [C.c_void_p, C.POINTER(C.c_double), C.POINTER(C.c_double)]),
     "pasta_particle_energies": (C.c_int, [C.c_void_p, C.c_void_p]),
     "pasta_pair_count": (C.c_int, [C.c_void_p, C.POINTER(C.c_int64)]),
+    "pasta_force_stats": (C.c_int, [C.c_void_p, C.POINTER(C.c_int64)]),
     "pasta_set_timing": (C.c_int, [C.c_void_p, C.c_int32]),
     "pasta_get_timing": (C.c_int, [C.c_void_p, C.POINTER(C.c_double), C.POINTER(C.c_int64)]),
     "pasta_launch_count": (C.c_int64, [C.c_void_p]),
@@ -298,6 +299,11 @@ class Sim:
         n = C.c_int64()
         _check(self.lib.pasta_pair_count(self._h, C.byref(n)))
         return n.value
+
+    def force_stats(self):
+        out = (C.c_int64 * 3)()
+        _check(self.lib.pasta_force_stats(self._h, out))
+        return {"raw_candidates": out[0], "queued_candidates": out[1], "pair_evaluations": out[2]}
 
     def set_timing(self, enable=True):
         _check(self.lib.pasta_set_timing(self._h, 1 if enable else 0))

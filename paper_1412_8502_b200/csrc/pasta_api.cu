@@ -221,7 +221,7 @@ int pasta_create(pasta_sim** out, int64_t N, double Y_P, double density, double 
         (rc = buffer_reserve(s, &s->is_p, n)) || (rc = buffer_reserve(s, &s->cell_id, 4 * n)) ||
         (rc = buffer_reserve(s, &s->perm, 4 * n)) || (rc = buffer_reserve(s, &s->pos4, 16 * n + 4096)) ||
         (rc = buffer_reserve(s, &s->cxyz, 4 * n)) || (rc = buffer_reserve(s, &s->partials, 8 * 8192)) ||
-        (rc = buffer_reserve(s, &s->scalars, 8 * 16)) || (rc = buffer_reserve(s, &s->counters, 8 * 16)))
+        (rc = buffer_reserve(s, &s->scalars, 8 * 16)) || (rc = buffer_reserve(s, &s->counters, 8 * 32)))
       break;
     if (cudaMemsetAsync(s->F.ptr, 0, 24 * n, s->stream) != cudaSuccess ||
         cudaMemsetAsync(s->e.ptr, 0, 8 * n, s->stream) != cudaSuccess ||
@@ -493,6 +493,26 @@ int pasta_pair_count(pasta_sim* sim, int64_t* ordered_pairs_host) {
   PASTA_TRY(use_device(s));
   PASTA_TRY(k1_build(s));
   return k2_pair_count(s, ordered_pairs_host);
+}
+
+int pasta_force_stats(pasta_sim* sim, int64_t* out3_host) {
+  Sim* s = reinterpret_cast<Sim*>(sim);
+  PASTA_TRY(check_sim(s));
+  if (!out3_host) {
+    set_error("out3_host is NULL");
+    return PASTA_EINVAL;
+  }
+  PASTA_TRY(use_device(s));
+  PASTA_TRY(k1_build(s));
+  PASTA_TRY(k2_chunk_forces(s, true, true));
+  s->forces_valid = true;
+  s->energies_valid = true;
+  unsigned long long h[3];
+  PASTA_CUDA_OK(cudaMemcpyAsync(h, s->counters.as<unsigned long long>() + 10, sizeof(h), cudaMemcpyDeviceToHost,
+                                s->stream));
+  PASTA_CUDA_OK(cudaStreamSynchronize(s->stream));
+  for (int k = 0; k < 3; ++k) out3_host[k] = (int64_t)h[k];
+  return PASTA_OK;
 }
 
 int pasta_set_timing(pasta_sim* sim, int32_t enable) {

@@ -120,6 +120,8 @@ int scan_exclusive(Sim* s, const int32_t* in, int32_t* out, int64_t n);  // out[
 // K2  k2_force.cu
 int k2_forces(Sim* s, bool with_energy);               // F, e in original order
 int k2_pair_count(Sim* s, int64_t* ordered_pairs_host);
+int k2_reference_forces(Sim* s, bool with_energy);     // variant 1: thread per target (k2_force.cu)
+int k2_chunk_forces(Sim* s, bool with_energy, bool stats);  // variant 2: chunk kernel (k2_chunk.cu)
 // K3  k3_integrate.cu
 int k3_init_state(Sim* s, uint64_t seed);
 int k3_kick_drift(Sim* s, double dt, double scale, double L_new);
