@@ -56,6 +56,9 @@ typedef struct pasta_params {
   int32_t cell_subdiv;         /* k >= 1: cells per side = max(1, floor(L k / r_c)), width L/ncell >= r_c/k (D14) */
   int32_t force_variant;       /* 0 = library default; >0 selects a specific pair-force kernel */
   int32_t energy_every_step;   /* 1 (default): pasta_step evaluates per-particle energies with the forces */
+  int32_t auto_grid;           /* 1 (default): each species' force grid picks its own k (about 8 particles per cell);
+                                  0: both use cell_subdiv.  pasta_cells always reports the cell_subdiv grid */
+  int32_t reserved1;
 } pasta_params;
 
 /* Device environment: where internal memory and the stream come from. */

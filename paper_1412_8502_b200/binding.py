@@ -28,7 +28,7 @@ class Params(C.Structure):
         ("alpha_hbarc", C.c_double), ("lambda_", C.c_double), ("r_c", C.c_double), ("mass", C.c_double),
         ("scale_per_step", C.c_double),
         ("thermostat_interval", C.c_int32), ("cell_subdiv", C.c_int32), ("force_variant", C.c_int32),
-        ("energy_every_step", C.c_int32),
+        ("energy_every_step", C.c_int32), ("auto_grid", C.c_int32), ("reserved1", C.c_int32),
     ]
 
 

@@ -1,13 +1,17 @@
 // K1 -- counting-sort cell list (cubical cells, here rebuilt
 // every step on the GPU instead of a halo'd neighbour list on the CPU).
 //
-// Layout produced (all in HBM, L2-resident at these sizes):
-//   cell_id[N]            O3 id (cz*ncell + cy)*ncell + cx of every particle, original order
-//   bin_start[2*nc3 + 1]  exclusive scan over (species, cell) bins; bin = (is_proton ? 0 : nc3) + id,
-//                         so sorted slots [0, Np) are protons and [Np, N) neutrons, each cell-sorted
+// Each species has its own grid (same O3 formula, its own k): grid[0] for protons, grid[1] for neutrons,
+// sized so that a cell holds about one chunk (8 particles) of that species -- chunks of the pair kernel
+// are then compact for both species.  Layout produced (all in HBM, L2-resident at these sizes):
+//   pbin[N]               bin of every particle, original order: base[species] + (cz*ncell + cy)*ncell + cx
+//   bin_start[nbins + 1]  exclusive scan over the bins; protons' bins come first, so sorted slots
+//                         [0, Np) are protons and [Np, N) neutrons, each sorted by its own grid's cell id
 //   perm[N]               sorted slot -> original index, ascending inside a bin (deterministic order)
 //   pos4[N]  (float4)     sigma * (x - cell centre) for x, y, z (|.| <= sigma w / 2)  and .w = (float)cx
 //   cxyz[N]               cx | cy << 10 | cz << 20
+// pasta_cells() exports the species-independent O3 grid of pasta_params.cell_subdiv with the same
+// cell_coord arithmetic.
 #include "pasta_internal.cuh"
 
 namespace pasta {
@@ -31,17 +35,38 @@ __device__ __forceinline__ int cell_coord(double x, double inv_w, int ncell) {
   return q < 0 ? 0 : q;
 }
 
+struct GridPair {
+  int ncell[2];
+  int base[2];  // first bin of the species' grid: base[0] = 0, base[1] = ncell[0]^3
+  double inv_w[2], w[2];
+};
+
 __global__ void k1_count_kernel(int64_t N, const double* __restrict__ x, const uint8_t* __restrict__ is_p,
-                                double inv_w, int ncell, int nc3, int32_t* __restrict__ cell_id,
-                                int32_t* __restrict__ bin_count) {
+                                const GridPair g, int32_t* __restrict__ pbin, int32_t* __restrict__ bin_count) {
+  int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= N) return;
+  const int sp = is_p[i] ? 0 : 1;
+  const int nc = g.ncell[sp];
+  const double iw = g.inv_w[sp];
+  int cx = cell_coord(x[3 * i + 0], iw, nc);
+  int cy = cell_coord(x[3 * i + 1], iw, nc);
+  int cz = cell_coord(x[3 * i + 2], iw, nc);
+  const int bin = g.base[sp] + (cz * nc + cy) * nc + cx;
+  pbin[i] = bin;
+  atomicAdd(&bin_count[bin], 1);
+}
+
+// O3 ids on the exported grid (species-independent), with the histogram for cell_start.
+__global__ void k1_o3_kernel(int64_t N, const double* __restrict__ x, double inv_w, int ncell,
+                             int32_t* __restrict__ cell_id, int32_t* __restrict__ count) {
   int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= N) return;
   int cx = cell_coord(x[3 * i + 0], inv_w, ncell);
   int cy = cell_coord(x[3 * i + 1], inv_w, ncell);
   int cz = cell_coord(x[3 * i + 2], inv_w, ncell);
-  int id = (cz * ncell + cy) * ncell + cx;
+  const int id = (cz * ncell + cy) * ncell + cx;
   cell_id[i] = id;
-  atomicAdd(&bin_count[(is_p[i] ? 0 : nc3) + id], 1);
+  atomicAdd(&count[id], 1);
 }
 
 // ---- exclusive scan: 2048 items per block, three small kernels ----------------------------------------
@@ -132,13 +157,12 @@ int scan_exclusive(Sim* s, const int32_t* in, int32_t* out, int64_t n) {
   return PASTA_OK;
 }
 
-__global__ void k1_scatter_kernel(int64_t N, const int32_t* __restrict__ cell_id, const uint8_t* __restrict__ is_p,
-                                  int nc3, const int32_t* __restrict__ bin_start, int32_t* __restrict__ bin_count,
-                                  int32_t* __restrict__ perm) {
+__global__ void k1_scatter_kernel(int64_t N, const int32_t* __restrict__ pbin, const int32_t* __restrict__ bin_start,
+                                  int32_t* __restrict__ bin_count, int32_t* __restrict__ perm) {
   int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= N) return;
-  int bin = (is_p[i] ? 0 : nc3) + cell_id[i];
-  int old = atomicSub(&bin_count[bin], 1);  // leaves the histogram zeroed for the next build
+  const int bin = pbin[i];
+  const int old = atomicSub(&bin_count[bin], 1);  // leaves the histogram zeroed for the next build
   perm[bin_start[bin] + old - 1] = (int32_t)i;
 }
 
@@ -158,14 +182,17 @@ __global__ void k1_order_kernel(int64_t nbins, const int32_t* __restrict__ bin_s
   }
 }
 
-__global__ void k1_gather_kernel(int64_t N, const double* __restrict__ x, const int32_t* __restrict__ cell_id,
-                                 const int32_t* __restrict__ perm, int ncell, double w, double sigma,
+__global__ void k1_gather_kernel(int64_t N, const double* __restrict__ x, const int32_t* __restrict__ pbin,
+                                 const int32_t* __restrict__ perm, const GridPair g, double sigma,
                                  float4* __restrict__ pos4, int32_t* __restrict__ cxyz) {
   int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (t >= N) return;
   const int i = perm[t];
-  const int id = cell_id[i];
-  const int cx = id % ncell, cy = (id / ncell) % ncell, cz = id / (ncell * ncell);
+  const int bin = pbin[i];
+  const int sp = bin >= g.base[1] ? 1 : 0;
+  const int id = bin - g.base[sp], nc = g.ncell[sp];
+  const double w = g.w[sp];
+  const int cx = id % nc, cy = (id / nc) % nc, cz = id / (nc * nc);
   float4 p;
   p.x = (float)(sigma * (x[3 * i + 0] - ((double)cx + 0.5) * w));
   p.y = (float)(sigma * (x[3 * i + 1] - ((double)cy + 0.5) * w));
@@ -175,51 +202,72 @@ __global__ void k1_gather_kernel(int64_t N, const double* __restrict__ x, const 
   cxyz[t] = cx | (cy << 10) | (cz << 20);
 }
 
-int k1_build(Sim* s) {
+// Cells per side of a species' grid: the O3 formula with the k that puts about CHUNK particles in a cell.
+static int auto_subdiv(double L, double r_c, int64_t n_species, int k_default) {
+  if (n_species <= 0) return k_default;
+  const double w_star = L * cbrt(8.0 / (double)n_species);
+  int k = (int)floor(r_c / w_star + 0.5);
+  return k < 1 ? 1 : (k > 64 ? 64 : k);
+}
+
+int k1_build(Sim* s, bool uniform_grid) {
   const int64_t N = s->N;
-  s->grid = make_grid(s->L, s->prm.r_c, s->prm.cell_subdiv);
-  const Grid& g = s->grid;
-  const int64_t nbins = 2 * g.nc3;
+  const bool uniform = uniform_grid || s->prm.auto_grid == 0 || s->prm.force_variant == 1;
+  const int k0 = uniform ? s->prm.cell_subdiv : auto_subdiv(s->L, s->prm.r_c, s->Np, s->prm.cell_subdiv);
+  const int k1 = uniform ? s->prm.cell_subdiv : auto_subdiv(s->L, s->prm.r_c, N - s->Np, s->prm.cell_subdiv);
+  s->grid_sp[0] = make_grid(s->L, s->prm.r_c, k0);
+  s->grid_sp[1] = make_grid(s->L, s->prm.r_c, k1);
+  GridPair g;
+  for (int sp = 0; sp < 2; ++sp) {
+    g.ncell[sp] = s->grid_sp[sp].ncell;
+    g.inv_w[sp] = s->grid_sp[sp].inv_w;
+    g.w[sp] = s->grid_sp[sp].w;
+  }
+  g.base[0] = 0;
+  g.base[1] = (int)s->grid_sp[0].nc3;
+  s->bin_base[0] = 0;
+  s->bin_base[1] = s->grid_sp[0].nc3;
+  const int64_t nbins = s->grid_sp[0].nc3 + s->grid_sp[1].nc3;
   PASTA_TRY(buffer_reserve(s, &s->bin_count, sizeof(int32_t) * (size_t)(nbins + 1)));
   PASTA_TRY(buffer_reserve(s, &s->bin_start, sizeof(int32_t) * (size_t)(nbins + 1)));
   int32_t* cnt = s->bin_count.as<int32_t>();
   int32_t* start = s->bin_start.as<int32_t>();
   PASTA_CUDA_OK(cudaMemsetAsync(cnt, 0, sizeof(int32_t) * (size_t)(nbins + 1), s->stream));
   const int B = 256;
-  k1_count_kernel<<<grid_for(N, B), B, 0, s->stream>>>(N, s->x.as<double>(), s->is_p.as<uint8_t>(), g.inv_w, g.ncell,
-                                                       (int)g.nc3, s->cell_id.as<int32_t>(), cnt);
+  k1_count_kernel<<<grid_for(N, B), B, 0, s->stream>>>(N, s->x.as<double>(), s->is_p.as<uint8_t>(), g,
+                                                       s->cell_id.as<int32_t>(), cnt);
   s->launches += 1;
   PASTA_TRY(scan_exclusive(s, cnt, start, nbins));
-  k1_scatter_kernel<<<grid_for(N, B), B, 0, s->stream>>>(N, s->cell_id.as<int32_t>(), s->is_p.as<uint8_t>(),
-                                                         (int)g.nc3, start, cnt, s->perm.as<int32_t>());
+  k1_scatter_kernel<<<grid_for(N, B), B, 0, s->stream>>>(N, s->cell_id.as<int32_t>(), start, cnt, s->perm.as<int32_t>());
   k1_order_kernel<<<grid_for(nbins, B), B, 0, s->stream>>>(nbins, start, s->perm.as<int32_t>());
   const double sigma = sqrt(1.4426950408889634074 / (2.0 * s->prm.Lambda));
   k1_gather_kernel<<<grid_for(N, B), B, 0, s->stream>>>(N, s->x.as<double>(), s->cell_id.as<int32_t>(),
-                                                        s->perm.as<int32_t>(), g.ncell, g.w, sigma,
-                                                        s->pos4.as<float4>(), s->cxyz.as<int32_t>());
+                                                        s->perm.as<int32_t>(), g, sigma, s->pos4.as<float4>(),
+                                                        s->cxyz.as<int32_t>());
   s->launches += 3;
   PASTA_CUDA_OK(cudaGetLastError());
   return PASTA_OK;
 }
 
-// cell_start of the species-independent O3 histogram, for pasta_cells: start_p[c] + (start_n[c] - Np).
-__global__ void k1_cell_start_kernel(int64_t nc3, const int32_t* __restrict__ bin_start, int32_t* __restrict__ out) {
-  int64_t c = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-  if (c > nc3) return;
-  const int np = bin_start[nc3];
-  out[c] = bin_start[c] + (bin_start[nc3 + c] - np);
-}
-
+// pasta_cells: the O3 grid of cell_subdiv, species-independent (uses the cell-list scratch buffers; the next
+// force evaluation rebuilds them anyway).
 int k1_export_cells(Sim* s, int32_t* cell_id_dev, int32_t* cell_start_dev) {
-  PASTA_TRY(k1_build(s));
+  const Grid g = make_grid(s->L, s->prm.r_c, s->prm.cell_subdiv);
+  PASTA_TRY(buffer_reserve(s, &s->bin_count, sizeof(int32_t) * (size_t)(g.nc3 + 1)));
+  PASTA_TRY(buffer_reserve(s, &s->bin_start, sizeof(int32_t) * (size_t)(g.nc3 + 1)));
+  int32_t* cnt = s->bin_count.as<int32_t>();
+  PASTA_CUDA_OK(cudaMemsetAsync(cnt, 0, sizeof(int32_t) * (size_t)(g.nc3 + 1), s->stream));
+  k1_o3_kernel<<<grid_for(s->N, 256), 256, 0, s->stream>>>(s->N, s->x.as<double>(), g.inv_w, g.ncell,
+                                                           s->cell_id.as<int32_t>(), cnt);
+  s->launches += 1;
+  PASTA_CUDA_OK(cudaGetLastError());
   if (cell_id_dev)
     PASTA_CUDA_OK(cudaMemcpyAsync(cell_id_dev, s->cell_id.ptr, sizeof(int32_t) * (size_t)s->N,
                                   cudaMemcpyDeviceToDevice, s->stream));
   if (cell_start_dev) {
-    k1_cell_start_kernel<<<grid_for(s->grid.nc3 + 1, 256), 256, 0, s->stream>>>(s->grid.nc3, s->bin_start.as<int32_t>(),
-                                                                              cell_start_dev);
-    s->launches += 1;
-    PASTA_CUDA_OK(cudaGetLastError());
+    PASTA_TRY(scan_exclusive(s, cnt, s->bin_start.as<int32_t>(), g.nc3));
+    PASTA_CUDA_OK(cudaMemcpyAsync(cell_start_dev, s->bin_start.ptr, sizeof(int32_t) * (size_t)(g.nc3 + 1),
+                                  cudaMemcpyDeviceToDevice, s->stream));
   }
   return PASTA_OK;
 }

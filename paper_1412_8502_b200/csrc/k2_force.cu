@@ -187,10 +187,10 @@ static V0Args make_v0_args(Sim* s) {
   V0Args A;
   A.N = s->N;
   A.Np = (int32_t)s->Np;
-  A.ncell = s->grid.ncell;
-  A.nc3 = (int32_t)s->grid.nc3;
+  A.ncell = s->grid_sp[0].ncell;  // both species share one grid for this kernel (k1_build uniform)
+  A.nc3 = (int32_t)s->grid_sp[0].nc3;
   A.k = s->prm.cell_subdiv;
-  A.wS = (float)(sigma * s->grid.w);
+  A.wS = (float)(sigma * s->grid_sp[0].w);
   A.LS = (float)(sigma * s->L);
   A.inv_LS = (float)(1.0 / (sigma * s->L));
   A.pos4 = s->pos4.as<float4>();

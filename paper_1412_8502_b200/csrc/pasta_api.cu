@@ -150,6 +150,7 @@ int pasta_params_default(pasta_params* p) {
   p->cell_subdiv = 4;
   p->force_variant = 0;
   p->energy_every_step = 1;
+  p->auto_grid = 1;
   return PASTA_OK;
 }
 
@@ -451,7 +452,7 @@ int pasta_cells(pasta_sim* sim, int32_t* cell_id_dev, int32_t* cell_start_dev, i
   PASTA_TRY(check_sim(s));
   PASTA_TRY(use_device(s));
   PASTA_TRY(k1_export_cells(s, cell_id_dev, cell_start_dev));
-  if (ncell_side_host) *ncell_side_host = s->grid.ncell;
+  if (ncell_side_host) *ncell_side_host = make_grid(s->L, s->prm.r_c, s->prm.cell_subdiv).ncell;
   return PASTA_OK;
 }
 
@@ -491,7 +492,7 @@ int pasta_pair_count(pasta_sim* sim, int64_t* ordered_pairs_host) {
     return PASTA_EINVAL;
   }
   PASTA_TRY(use_device(s));
-  PASTA_TRY(k1_build(s));
+  PASTA_TRY(k1_build(s, true));  // the counting kernel walks one common grid
   return k2_pair_count(s, ordered_pairs_host);
 }
 

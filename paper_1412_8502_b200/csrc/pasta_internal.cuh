@@ -82,8 +82,9 @@ struct Sim {
   Buffer x, v, F, e, is_p;  // double[N][3] x3, double[N], uint8[N]
 
   // cell list (device)
-  Grid grid;
-  Buffer cell_id;     // int32[N]   O3 id (species-independent)
+  Grid grid_sp[2];    // [0] protons' grid, [1] neutrons' grid
+  int64_t bin_base[2] = {0, 0};
+  Buffer cell_id;     // int32[N]   bin of every particle (force grids) / O3 id (pasta_cells)
   Buffer bin_count;   // int32[2 nc3 + 1] scratch histogram over (species, cell) bins
   Buffer bin_start;   // int32[2 nc3 + 1] exclusive scan; protons' bins first
   Buffer scan_tmp;    // block sums of the scan
@@ -114,7 +115,7 @@ struct Sim {
 
 // ---- kernel launchers (one translation unit each) ---------------------------------------------------
 // K1  k1_cells.cu
-int k1_build(Sim* s);                                  // cell ids, (species,cell) counting sort, pos4/perm
+int k1_build(Sim* s, bool uniform_grid = false);                                // cell ids, (species,cell) counting sort, pos4/perm
 int k1_export_cells(Sim* s, int32_t* cell_id_dev, int32_t* cell_start_dev);
 int scan_exclusive(Sim* s, const int32_t* in, int32_t* out, int64_t n);  // out[0..n] (n+1 entries)
 // K2  k2_force.cu

