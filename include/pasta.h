@@ -58,7 +58,7 @@ typedef struct pasta_params {
   int32_t energy_every_step;   /* 1 (default): pasta_step evaluates per-particle energies with the forces */
   int32_t auto_grid;           /* 1 (default): each species' force grid picks its own k (about 8 particles per cell);
                                   0: both use cell_subdiv.  pasta_cells always reports the cell_subdiv grid */
-  int32_t reserved1;
+  int32_t x_subdiv;            /* thin cells along x per force-grid cell (0 = library default, 4) */
 } pasta_params;
 
 /* Device environment: where internal memory and the stream come from. */
@@ -161,9 +161,9 @@ int pasta_particle_energies(pasta_sim* sim, double* e_dev);
  * kernel in the same FP32 arithmetic the force kernel uses: the work unit of the throughput metric. */
 int pasta_pair_count(pasta_sim* sim, int64_t* ordered_pairs_host);
 
-/* Work statistics of one evaluation with the chunk pair kernel: out3_host = {raw candidates streamed from
- * the cell rows, candidates that survived the bounding-sphere test, pair evaluations executed}.
- * Synchronises.  (ordered in-range pairs / pair evaluations = the kernel's useful-work fraction.) */
+/* Work statistics of one evaluation with the chunk pair kernel: out3_host = {sources streamed from the cell
+ * rows (summed over chunks), tiles of <= 32 sources, pair evaluations executed}.  Synchronises.
+ * (ordered in-range pairs / pair evaluations = the kernel's useful-work fraction.) */
 int pasta_force_stats(pasta_sim* sim, int64_t* out3_host);
 
 /*

@@ -28,7 +28,7 @@ class Params(C.Structure):
         ("alpha_hbarc", C.c_double), ("lambda_", C.c_double), ("r_c", C.c_double), ("mass", C.c_double),
         ("scale_per_step", C.c_double),
         ("thermostat_interval", C.c_int32), ("cell_subdiv", C.c_int32), ("force_variant", C.c_int32),
-        ("energy_every_step", C.c_int32), ("auto_grid", C.c_int32), ("reserved1", C.c_int32),
+        ("energy_every_step", C.c_int32), ("auto_grid", C.c_int32), ("x_subdiv", C.c_int32),
     ]
 
 
@@ -303,7 +303,7 @@ class Sim:
     def force_stats(self):
         out = (C.c_int64 * 3)()
         _check(self.lib.pasta_force_stats(self._h, out))
-        return {"raw_candidates": out[0], "queued_candidates": out[1], "pair_evaluations": out[2]}
+        return {"sources_streamed": out[0], "tiles": out[1], "pair_evaluations": out[2]}
 
     def set_timing(self, enable=True):
         _check(self.lib.pasta_set_timing(self._h, 1 if enable else 0))

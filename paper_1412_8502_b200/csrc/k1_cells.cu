@@ -9,22 +9,27 @@
 //                         [0, Np) are protons and [Np, N) neutrons, each sorted by its own grid's cell id
 //   perm[N]               sorted slot -> original index, ascending inside a bin (deterministic order)
 //   pos4[N]  (float4)     sigma * (x - cell centre) for x, y, z (|.| <= sigma w / 2)  and .w = (float)cx
-//   cxyz[N]               cx | cy << 10 | cz << 20
+//   cxyz[N]               cx | cy << 12 | cz << 22
 // pasta_cells() exports the species-independent O3 grid of pasta_params.cell_subdiv with the same
 // cell_coord arithmetic.
 #include "pasta_internal.cuh"
 
 namespace pasta {
 
-Grid make_grid(double L, double r_c, int32_t k) {
+Grid make_grid(double L, double r_c, int32_t k, int32_t xsub) {
   Grid g;
   double q = floor(L * (double)k / r_c);
   if (q < 1.0) q = 1.0;
-  if (q > 1023.0) q = 1023.0;  // cx, cy, cz are packed in 10 bits each
+  if (q > 1023.0) q = 1023.0;  // cy, cz are packed in 10 bits each, cx in 12
   g.ncell = (int32_t)q;
-  g.nc3 = (int64_t)g.ncell * g.ncell * g.ncell;
+  g.xsub = xsub < 1 ? 1 : xsub;
+  while (g.ncell * g.xsub > 4095) g.xsub -= 1;
+  g.ncx = g.ncell * g.xsub;
+  g.nc3 = (int64_t)g.ncell * g.ncell * g.ncx;
   g.inv_w = (double)g.ncell / L;
   g.w = L / (double)g.ncell;
+  g.inv_wx = (double)g.ncx / L;
+  g.wx = L / (double)g.ncx;
   return g;
 }
 
@@ -36,9 +41,9 @@ __device__ __forceinline__ int cell_coord(double x, double inv_w, int ncell) {
 }
 
 struct GridPair {
-  int ncell[2];
-  int base[2];  // first bin of the species' grid: base[0] = 0, base[1] = ncell[0]^3
-  double inv_w[2], w[2];
+  int ncell[2], ncx[2];
+  int base[2];  // first bin of the species' grid: base[0] = 0, base[1] = number of cells of grid 0
+  double inv_w[2], w[2], inv_wx[2], wx[2];
 };
 
 __global__ void k1_count_kernel(int64_t N, const double* __restrict__ x, const uint8_t* __restrict__ is_p,
@@ -46,12 +51,12 @@ __global__ void k1_count_kernel(int64_t N, const double* __restrict__ x, const u
   int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= N) return;
   const int sp = is_p[i] ? 0 : 1;
-  const int nc = g.ncell[sp];
+  const int nc = g.ncell[sp], ncx = g.ncx[sp];
   const double iw = g.inv_w[sp];
-  int cx = cell_coord(x[3 * i + 0], iw, nc);
+  int cx = cell_coord(x[3 * i + 0], g.inv_wx[sp], ncx);
   int cy = cell_coord(x[3 * i + 1], iw, nc);
   int cz = cell_coord(x[3 * i + 2], iw, nc);
-  const int bin = g.base[sp] + (cz * nc + cy) * nc + cx;
+  const int bin = g.base[sp] + (cz * nc + cy) * ncx + cx;
   pbin[i] = bin;
   atomicAdd(&bin_count[bin], 1);
 }
@@ -190,16 +195,16 @@ __global__ void k1_gather_kernel(int64_t N, const double* __restrict__ x, const 
   const int i = perm[t];
   const int bin = pbin[i];
   const int sp = bin >= g.base[1] ? 1 : 0;
-  const int id = bin - g.base[sp], nc = g.ncell[sp];
+  const int id = bin - g.base[sp], nc = g.ncell[sp], ncx = g.ncx[sp];
   const double w = g.w[sp];
-  const int cx = id % nc, cy = (id / nc) % nc, cz = id / (nc * nc);
+  const int cx = id % ncx, cy = (id / ncx) % nc, cz = id / (ncx * nc);
   float4 p;
-  p.x = (float)(sigma * (x[3 * i + 0] - ((double)cx + 0.5) * w));
+  p.x = (float)(sigma * (x[3 * i + 0] - ((double)cx + 0.5) * g.wx[sp]));
   p.y = (float)(sigma * (x[3 * i + 1] - ((double)cy + 0.5) * w));
   p.z = (float)(sigma * (x[3 * i + 2] - ((double)cz + 0.5) * w));
   p.w = (float)cx;
   pos4[t] = p;
-  cxyz[t] = cx | (cy << 10) | (cz << 20);
+  cxyz[t] = cx | (cy << 12) | (cz << 22);
 }
 
 // Cells per side of a species' grid: the O3 formula with the k that puts about CHUNK particles in a cell.
@@ -212,16 +217,23 @@ static int auto_subdiv(double L, double r_c, int64_t n_species, int k_default) {
 
 int k1_build(Sim* s, bool uniform_grid) {
   const int64_t N = s->N;
-  const bool uniform = uniform_grid || s->prm.auto_grid == 0 || s->prm.force_variant == 1;
-  const int k0 = uniform ? s->prm.cell_subdiv : auto_subdiv(s->L, s->prm.r_c, s->Np, s->prm.cell_subdiv);
-  const int k1 = uniform ? s->prm.cell_subdiv : auto_subdiv(s->L, s->prm.r_c, N - s->Np, s->prm.cell_subdiv);
-  s->grid_sp[0] = make_grid(s->L, s->prm.r_c, k0);
-  s->grid_sp[1] = make_grid(s->L, s->prm.r_c, k1);
+  // the reference kernel and the pair counter walk ONE isotropic grid; the chunk kernel takes a grid per
+  // species, each cell sliced into thin cells along x (rows sorted in x: tight source ranges, compact chunks)
+  const bool uniform = uniform_grid || s->prm.force_variant == 1;
+  const bool same_k = uniform || s->prm.auto_grid == 0;
+  const int k0 = same_k ? s->prm.cell_subdiv : auto_subdiv(s->L, s->prm.r_c, s->Np, s->prm.cell_subdiv);
+  const int k1 = same_k ? s->prm.cell_subdiv : auto_subdiv(s->L, s->prm.r_c, N - s->Np, s->prm.cell_subdiv);
+  const int xsub = uniform ? 1 : (s->prm.x_subdiv > 0 ? s->prm.x_subdiv : 4);
+  s->grid_sp[0] = make_grid(s->L, s->prm.r_c, k0, xsub);
+  s->grid_sp[1] = make_grid(s->L, s->prm.r_c, k1, xsub);
   GridPair g;
   for (int sp = 0; sp < 2; ++sp) {
     g.ncell[sp] = s->grid_sp[sp].ncell;
+    g.ncx[sp] = s->grid_sp[sp].ncx;
     g.inv_w[sp] = s->grid_sp[sp].inv_w;
     g.w[sp] = s->grid_sp[sp].w;
+    g.inv_wx[sp] = s->grid_sp[sp].inv_wx;
+    g.wx[sp] = s->grid_sp[sp].wx;
   }
   g.base[0] = 0;
   g.base[1] = (int)s->grid_sp[0].nc3;

@@ -1,26 +1,25 @@
 // K2, production variant -- "chunk" pair-force kernel for sm_100a.
 //
 // Work decomposition:
-//   * a CHUNK is T = 8 consecutive same-species particles of the cell-sorted order (about one cell of that
-//     species' grid, so it is spatially compact); one warp owns one chunk.  The 8 targets live in
+//   * a CHUNK is T = 8 consecutive same-species particles of the cell-sorted order.  The force grids are
+//     sliced into thin cells along x, so a row of cells (fixed cy, cz) is sorted in x and a chunk is a
+//     short stretch of one row: spatially compact.  One warp owns one chunk.  The 8 targets live in
 //     registers, replicated in every lane and packed two by two, so that the pair arithmetic runs as
-//     packed FP32 (FFMA2/FADD2/FMUL2: two pairs per issued instruction -- the FMA pipe, not the issue
-//     port, is then the binding unit).
-//   * LANES run over SOURCES.  For each source species the warp lists the rows of cells (fixed cy, cz)
-//     of that species' grid that intersect the chunk's bounding sphere inflated by r_c; a row's cells
-//     are contiguous in the sorted arrays, so a row is one segment of slots (two where it crosses the
-//     periodic boundary: images are enumerated explicitly, there is no per-pair nearest-image
-//     arithmetic and small boxes need no special case).
-//   * the segments are streamed 32 slots at a time through a 4-deep cp.async ring (global -> shared,
-//     no registers), so the L2 latency of the position loads is off the critical path.
-//   * every lane tests its source against the inflated sphere and the survivors are compacted through
-//     a 64-entry shared-memory ring (ballot + popc); whenever 32 survivors are queued, each lane takes
-//     one and evaluates it against all 8 targets.  The expensive part therefore runs on dense warps
-//     although only ~45 % of the raw candidates of a cell stencil lie inside the sphere.
+//     packed FP32 (FFMA2/FADD2/FMUL2: two pairs per issued instruction).
+//   * LANES run over SOURCES.  For each source species the warp lists the rows of that species' grid
+//     that can hold a particle within r_c of the chunk's bounding box, and for every row the tight range
+//     of thin cells [lo_x - xr, hi_x + xr]; a range is contiguous in the sorted arrays, i.e. one segment
+//     of slots (two where it crosses the periodic boundary: images are enumerated explicitly, there is
+//     no per-pair nearest-image arithmetic and small boxes need no special case).  Segments are cut into
+//     TILES of <= 32 slots described by 16 bytes in shared memory.
+//   * tiles are streamed through a 4-deep cp.async ring (global -> shared, no registers), so the L2
+//     latency of the position loads is off the critical path; every lane takes one source of the tile
+//     and evaluates it against all 8 targets.  There is NO per-candidate test and no divergence: a
+//     source that is out of range of a target contributes exactly zero (next point).
 //   * the cut-off needs no test for np/nn pairs when sigma^2 r_c^2 > 126: exp2(-r'^2) flushes to exactly
 //     zero there, so out-of-range pairs contribute exactly 0 (D1: plain truncation).  pp pairs carry the
 //     screened Coulomb term and are cut explicitly; small r_c selects the explicitly cut path.
-//   * per-lane partial sums are FP32 (about 130 terms per target and pass); they are combined across
+//   * per-lane partial sums are FP32 (about 70 terms per target and pass); they are combined across
 //     lanes and passes in FP64 by a transposing butterfly, and written in original particle order.
 #include "pasta_internal.cuh"
 
@@ -32,7 +31,8 @@ constexpr int T = 8;            // targets per chunk
 constexpr int NP = T / 2;       // packed target pairs
 constexpr int WARPS = 4;        // warps (= chunks) per block
 constexpr int DEPTH = 4;        // cp.async stages per warp
-constexpr int SEG_CAP = 160;    // segment descriptors per warp
+constexpr int TILE_CAP = 512;   // tile descriptors per warp
+constexpr int EMIT_MAX = 8;     // tiles one lane may add per emission round (32 * 8 = half the table)
 constexpr float FAR = 1.0e10f;  // coordinate of padding sources/targets: exp2(-FAR^2) == 0, 0 * FAR == 0
 
 __device__ __forceinline__ float ex2_approx(float x) {
@@ -59,9 +59,10 @@ __device__ __forceinline__ void cp_async_wait() {
 }
 
 struct SpeciesGrid {
-  int32_t ncell, base;  // cells per side, first bin
-  float wS, inv_wS;     // sigma * cell width and its inverse
-  double wS_d;          // the same in FP64 (frame shifts between the two grids)
+  int32_t ncell, ncx, base;  // cells per side in y/z, thin cells per side in x, first bin
+  float wS, inv_wS;          // sigma * cell width (y, z) and its inverse
+  float wxS, inv_wxS;        // sigma * thin-cell width (x) and its inverse
+  double wS_d, wxS_d;        // the widths in FP64 (frame shifts between the two grids)
 };
 
 struct ChunkArgs {
@@ -75,20 +76,17 @@ struct ChunkArgs {
   const int32_t* perm;
   double* F;
   double* e;
-  unsigned long long* stats;  // [0] raw candidates, [1] queued candidates, [2] pair evaluations (STATS only)
+  unsigned long long* stats;  // [0] sources streamed, [1] tiles, [2] pair evaluations (STATS only)
 };
 
-struct __align__(16) Segment {  // slots [start, start + len): one periodic image of part of a row of cells
-  int start, len;
-  float xoff;  // add to pos4.w (cell x index) to get the cell offset from the frame's reference cell
-  float my, mz;  // cell offsets of the row from the reference cell
-  int pad[3];
-};
+// <= 32 consecutive slots of one periodic image of a row: x = (start << 6) | (count - 1); y = xoff (add to
+// pos4.w, the thin-cell index, to get the cell offset from the frame's reference cell); z, w = the row's
+// y and z offsets from the reference cell centre, already multiplied by the cell width.
+typedef float4 Tile;
 
 struct WarpShared {
-  float4 ring[64];
   float4 stage[DEPTH][32];
-  Segment seg[SEG_CAP];
+  Tile tile[TILE_CAP];
 };
 
 // Targets and accumulators of one warp.  Targets are replicated in all lanes; accumulators hold this
@@ -142,163 +140,139 @@ __device__ __forceinline__ void evaluate(const float4 s, const Targets& t, Accum
   }
 }
 
+
 __device__ __forceinline__ int floor_div(int a, int b) {  // b > 0
   const int q = a / b;
   return (a % b < 0) ? q - 1 : q;
 }
 
-// State of the compaction ring and of the frame of one pass.
-struct Frame {
-  float cX, cY, cZ, R2;  // bounding sphere (centre, inflated radius squared) of the chunk in this frame
-  float wS;              // sigma * cell width of the source grid
-};
-
-// Stream the listed segments: stage 32 slots at a time through the cp.async ring, test, compact into the
-// survivor ring, evaluate 32 survivors whenever they are available.
+// Stream the listed tiles through the cp.async ring and evaluate every source against the 8 targets.
 template <bool COUL, bool CUT, bool ENERGY, bool STATS>
-__device__ __forceinline__ void run_segments(const ChunkArgs& A, const PairConsts& c, WarpShared& sh, const int lane,
-                                             const int nseg, const int ntiles, const Frame& f, const Targets& t,
-                                             Accum& acc, const PassConsts& k, int& head, int& tail,
-                                             unsigned long long* st) {
-  if (nseg == 0) return;
-  const unsigned lt_mask = (1u << lane) - 1u;
-  // prefetch cursor
-  int ps = 0, po = 0;
-  int p_start = sh.seg[0].start, p_len = sh.seg[0].len;
-  auto issue = [&](int slot) {
-    const bool live = ps < nseg;
-    const bool in = live && (po + lane < p_len);
-    cp_async16(&sh.stage[slot][lane], A.pos4 + (in ? p_start + po + lane : 0), in ? 16 : 0);
-    cp_async_commit();
-    if (live) {
-      po += 32;
-      if (po >= p_len) {
-        ++ps;
-        po = 0;
-        if (ps < nseg) {
-          p_start = sh.seg[ps].start;
-          p_len = sh.seg[ps].len;
-        }
+__device__ __forceinline__ void run_tiles(const ChunkArgs& A, const PairConsts& c, WarpShared& sh, const int lane,
+                                          const int ntile, const float wxS, const Targets& t, Accum& acc,
+                                          const PassConsts& k, unsigned long long* st) {
+  if (ntile == 0) return;
+  auto issue = [&](int j, int slot) {
+    int src = 0, bytes = 0;
+    if (j < ntile) {
+      const unsigned d = __float_as_uint(sh.tile[j].x);
+      if (lane <= (int)(d & 63u)) {
+        src = (int)(d >> 6) + lane;
+        bytes = 16;
       }
     }
+    cp_async16(&sh.stage[slot][lane], A.pos4 + src, bytes);
+    cp_async_commit();
   };
 #pragma unroll
-  for (int d = 0; d < DEPTH; ++d) issue(d);
-
-  int cs = 0, co = 0;
-  Segment g = sh.seg[0];
-  for (int i = 0; i < ntiles; ++i) {
+  for (int d = 0; d < DEPTH; ++d) issue(d, d);
+  for (int i = 0; i < ntile; ++i) {
     cp_async_wait<DEPTH - 1>();
     const int slot = i & (DEPTH - 1);
     const float4 q = sh.stage[slot][lane];
-    const bool valid = co + lane < g.len;
-    // source position in the frame: cell-relative coordinate + integer cell offset * w'
-    const float X = fmaf(q.w + g.xoff, f.wS, q.x), Y = fmaf(g.my, f.wS, q.y), Z = fmaf(g.mz, f.wS, q.z);
-    const float dx = X - f.cX, dy = Y - f.cY, dz = Z - f.cZ;
-    const bool pass = valid && fmaf(dz, dz, fmaf(dy, dy, dx * dx)) < f.R2;
-    issue(slot);  // refill the stage just read (q has been consumed above)
-    const unsigned pm = __ballot_sync(0xffffffffu, pass);
-    if (pass) sh.ring[(tail + __popc(pm & lt_mask)) & 63] = make_float4(X, Y, Z, 0.f);
-    tail += __popc(pm);
+    const Tile tl = sh.tile[i];
+    const int cnt1 = (int)(__float_as_uint(tl.x) & 63u);
+    // source position in the frame: cell-relative coordinate + integer cell offset * cell width
+    float4 s;
+    s.x = fmaf(q.w + tl.y, wxS, q.x);
+    s.y = __fadd_rn(q.y, tl.z);
+    s.z = __fadd_rn(q.z, tl.w);
+    s.w = 0.f;
+    if (lane > cnt1) s.x = FAR;  // idle lanes of a short tile: a far-away source contributes exactly zero
+    issue(i + DEPTH, slot);      // refill the stage just read (q has been consumed above)
+    evaluate<COUL, CUT, ENERGY>(s, t, acc, k, c);
     if (STATS && lane == 0) {
-      st[0] += (unsigned long long)min(32, g.len - co);
-      st[1] += (unsigned long long)__popc(pm);
-    }
-    co += 32;
-    if (co >= g.len) {
-      ++cs;
-      co = 0;
-      if (cs < nseg) g = sh.seg[cs];
-    }
-    __syncwarp();
-    if (tail - head >= 32) {
-      const float4 cnd = sh.ring[(head + lane) & 63];
-      head += 32;
-      evaluate<COUL, CUT, ENERGY>(cnd, t, acc, k, c);
-      if (STATS && lane == 0) st[2] += 32ull * T;
-      __syncwarp();
+      st[0] += (unsigned long long)(cnt1 + 1);
+      st[1] += 1ull;
+      st[2] += 32ull * T;
     }
   }
   cp_async_wait<0>();
 }
 
-// One pass of a chunk over one source species.
+// Bounding box of the chunk in the frame of a pass.
+struct Box {
+  float lo_x, hi_x, lo_y, hi_y, lo_z, hi_z;
+};
+
+// One pass of a chunk over one source species: list the tiles, stream them.
 template <bool COUL, bool CUT, bool ENERGY, bool STATS>
 __device__ __forceinline__ void source_pass(const ChunkArgs& A, const PairConsts& c, WarpShared& sh, const int lane,
                                             const SpeciesGrid& gs, const int rx, const int ry, const int rz,
-                                            const Frame& f, const float R, const Targets& t, Accum& acc,
-                                            const PassConsts& k, unsigned long long* st) {
+                                            const Box& b, const Targets& t, Accum& acc, const PassConsts& k,
+                                            unsigned long long* st) {
   const float half = 0.5f * gs.wS;
-  // rows of cells (my, mz) whose slab can intersect the sphere; a hair of slack covers FP32 rounding of the
-  // cell-relative coordinates (every candidate is tested individually, so slack costs nothing but time)
+  // a hair of slack covers FP32 rounding of cell-relative coordinates against the cell boundaries
   const float slack = 1.0e-3f * gs.wS;
-  const int my_lo = (int)floorf((f.cY - R - slack) * gs.inv_wS + 0.5f), my_hi = (int)floorf((f.cY + R + slack) * gs.inv_wS + 0.5f);
-  const int mz_lo = (int)floorf((f.cZ - R - slack) * gs.inv_wS + 0.5f), mz_hi = (int)floorf((f.cZ + R + slack) * gs.inv_wS + 0.5f);
+  const float rc = A.rcS + slack, rc2 = rc * rc;
+  const int my_lo = (int)floorf((b.lo_y - rc) * gs.inv_wS + 0.5f), my_hi = (int)floorf((b.hi_y + rc) * gs.inv_wS + 0.5f);
+  const int mz_lo = (int)floorf((b.lo_z - rc) * gs.inv_wS + 0.5f), mz_hi = (int)floorf((b.hi_z + rc) * gs.inv_wS + 0.5f);
   const int ny = my_hi - my_lo + 1, nrows = ny * (mz_hi - mz_lo + 1);
-  const unsigned lt_mask = (1u << lane) - 1u;
-  const int nc = gs.ncell;
-  int head = 0, tail = 0;
-  int nseg_list = 0, ntiles = 0;
+  const int nc = gs.ncell, ncx = gs.ncx;
+  int ntile = 0;
 
   for (int rbase = 0; rbase < nrows; rbase += 32) {
     const int r = rbase + lane;
     int nseg = 0, ax_lo = 0, ax_hi = 0, q_lo = 0, rowbase = 0;
-    float myf = 0.f, mzf = 0.f;
+    float yoff = 0.f, zoff = 0.f;
     if (r < nrows) {
       const int my = my_lo + r % ny, mz = mz_lo + r / ny;
-      myf = (float)my;
-      mzf = (float)mz;
-      const float gy = fmaxf(fabsf(f.cY - myf * gs.wS) - half - slack, 0.f);
-      const float gz = fmaxf(fabsf(f.cZ - mzf * gs.wS) - half - slack, 0.f);
-      const float rem = f.R2 - gy * gy - gz * gz;
+      yoff = __fmul_rn((float)my, gs.wS);
+      zoff = __fmul_rn((float)mz, gs.wS);
+      // gap between the row's slab [off - w/2, off + w/2] and the box interval, per axis
+      const float gy = fmaxf(fmaxf(b.lo_y - (yoff + half), (yoff - half) - b.hi_y), 0.f);
+      const float gz = fmaxf(fmaxf(b.lo_z - (zoff + half), (zoff - half) - b.hi_z), 0.f);
+      const float rem = rc2 - gy * gy - gz * gz;
       if (rem > 0.f) {
-        const float xr = sqrtf(rem) + slack;
-        ax_lo = rx + (int)floorf((f.cX - xr) * gs.inv_wS + 0.5f);
-        ax_hi = rx + (int)floorf((f.cX + xr) * gs.inv_wS + 0.5f);
-        q_lo = floor_div(ax_lo, nc);
-        nseg = floor_div(ax_hi, nc) - q_lo + 1;
+        const float xr = sqrtf(rem);
+        ax_lo = rx + (int)floorf((b.lo_x - xr) * gs.inv_wxS + 0.5f);
+        ax_hi = rx + (int)floorf((b.hi_x + xr) * gs.inv_wxS + 0.5f);
+        q_lo = floor_div(ax_lo, ncx);
+        nseg = floor_div(ax_hi, ncx) - q_lo + 1;
         int ay = (ry + my) % nc, az = (rz + mz) % nc;
         ay += ay < 0 ? nc : 0;
         az += az < 0 ? nc : 0;
-        rowbase = gs.base + (az * nc + ay) * nc;
+        rowbase = gs.base + (az * nc + ay) * ncx;
       }
     }
     for (int round = 0; __any_sync(0xffffffffu, round < nseg); ++round) {
-      if (nseg_list + 32 > SEG_CAP) {  // (warp-uniform) list full: stream what is there
-        __syncwarp();
-        run_segments<COUL, CUT, ENERGY, STATS>(A, c, sh, lane, nseg_list, ntiles, f, t, acc, k, head, tail, st);
-        nseg_list = 0;
-        ntiles = 0;
-        __syncwarp();
+      int start = 0, len = 0;
+      float xoff = 0.f;
+      if (round < nseg) {
+        const int q = q_lo + round, qb = q * ncx;
+        const int a_lo = max(ax_lo, qb) - qb, a_hi = min(ax_hi, qb + ncx - 1) - qb;
+        start = __ldg(A.bin_start + rowbase + a_lo);
+        len = __ldg(A.bin_start + rowbase + a_hi + 1) - start;
+        xoff = (float)(qb - rx);
       }
-      bool has = round < nseg;
-      Segment sg;
-      sg.start = 0;
-      sg.len = 0;
-      if (has) {
-        const int q = q_lo + round, qb = q * nc;
-        const int a_lo = max(ax_lo, qb) - qb, a_hi = min(ax_hi, qb + nc - 1) - qb;
-        sg.start = __ldg(A.bin_start + rowbase + a_lo);
-        sg.len = __ldg(A.bin_start + rowbase + a_hi + 1) - sg.start;
-        sg.xoff = (float)(qb - rx);
-        sg.my = myf;
-        sg.mz = mzf;
-        has = sg.len > 0;
+      // emit the segment's tiles, at most EMIT_MAX per lane and round trip, so the table never overflows
+      while (__any_sync(0xffffffffu, len > 0)) {
+        if (ntile + 32 * EMIT_MAX > TILE_CAP) {  // (warp-uniform) table nearly full: stream what is there
+          __syncwarp();
+          run_tiles<COUL, CUT, ENERGY, STATS>(A, c, sh, lane, ntile, gs.wxS, t, acc, k, st);
+          ntile = 0;
+          __syncwarp();
+        }
+        const int mine = min((len + 31) >> 5, EMIT_MAX);
+        int incl = mine;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+          const int v = __shfl_up_sync(0xffffffffu, incl, o);
+          if (lane >= o) incl += v;
+        }
+        int at = ntile + incl - mine;
+        for (int m = 0; m < mine; ++m) {
+          const int cnt = min(len, 32);
+          sh.tile[at++] = make_float4(__uint_as_float(((unsigned)start << 6) | (unsigned)(cnt - 1)), xoff, yoff, zoff);
+          start += cnt;
+          len -= cnt;
+        }
+        ntile += __shfl_sync(0xffffffffu, incl, 31);
       }
-      const unsigned m = __ballot_sync(0xffffffffu, has);
-      if (has) sh.seg[nseg_list + __popc(m & lt_mask)] = sg;
-      nseg_list += __popc(m);
-      ntiles += __reduce_add_sync(0xffffffffu, has ? (sg.len + 31) >> 5 : 0);
     }
   }
   __syncwarp();
-  run_segments<COUL, CUT, ENERGY, STATS>(A, c, sh, lane, nseg_list, ntiles, f, t, acc, k, head, tail, st);
-  if (tail > head) {  // drain the ring; idle lanes take a far-away source that contributes exactly zero
-    float4 cnd = sh.ring[(head + lane) & 63];
-    if (head + lane >= tail) cnd = make_float4(FAR, FAR, FAR, 0.f);
-    evaluate<COUL, CUT, ENERGY>(cnd, t, acc, k, c);
-    if (STATS && lane == 0) st[2] += 32ull * T;
-  }
+  run_tiles<COUL, CUT, ENERGY, STATS>(A, c, sh, lane, ntile, gs.wxS, t, acc, k, st);
   __syncwarp();
 }
 
@@ -342,11 +316,11 @@ __global__ void __launch_bounds__(WARPS * 32, 3) k2_chunk_kernel(const ChunkArgs
   const float4 tp = __ldg(A.pos4 + base + tl);
   const int tc = __ldg(A.cxyz + base + tl);
   const int oc = __shfl_sync(0xffffffffu, tc, 0);
-  const int ox = oc & 1023, oy = (oc >> 10) & 1023, oz = (oc >> 20) & 1023;
+  const int ox = PASTA_CX(oc), oy = PASTA_CY(oc), oz = PASTA_CZ(oc);
   // cell offset from the origin cell, taken in the nearest periodic image (chunks may wrap a row end)
-  const int mx = min_image_cells((tc & 1023) - ox, gt.ncell);
-  const int my = min_image_cells(((tc >> 10) & 1023) - oy, gt.ncell);
-  const int mz = min_image_cells(((tc >> 20) & 1023) - oz, gt.ncell);
+  const int mx = min_image_cells(PASTA_CX(tc) - ox, gt.ncx);
+  const int my = min_image_cells(PASTA_CY(tc) - oy, gt.ncell);
+  const int mz = min_image_cells(PASTA_CZ(tc) - oz, gt.ncell);
 
   Accum acc;
 #pragma unroll
@@ -362,41 +336,30 @@ __global__ void __launch_bounds__(WARPS * 32, 3) k2_chunk_kernel(const ChunkArgs
     // itself at d == 0 exactly).  Other grid: the shift between the two cell centres is taken in FP64.
     int rx = ox, ry = oy, rz = oz;
     float X, Y, Z;
-    if (gs.ncell == gt.ncell) {  // same grid geometry (always true for the chunk's own species)
-      X = fmaf((float)mx, gs.wS, tp.x);
-      Y = fmaf((float)my, gs.wS, tp.y);
-      Z = fmaf((float)mz, gs.wS, tp.z);
+    if (gs.ncell == gt.ncell && gs.ncx == gt.ncx) {  // same grid geometry (always true for the chunk's own species)
+      X = fmaf((float)mx, gs.wxS, tp.x);
+      Y = __fadd_rn(tp.y, __fmul_rn((float)my, gs.wS));
+      Z = __fadd_rn(tp.z, __fmul_rn((float)mz, gs.wS));
     } else {
-      const double cx0 = ((double)ox + 0.5) * gt.wS_d, cy0 = ((double)oy + 0.5) * gt.wS_d, cz0 = ((double)oz + 0.5) * gt.wS_d;
-      rx = min(gs.ncell - 1, (int)(cx0 / gs.wS_d));
+      const double cx0 = ((double)ox + 0.5) * gt.wxS_d, cy0 = ((double)oy + 0.5) * gt.wS_d, cz0 = ((double)oz + 0.5) * gt.wS_d;
+      rx = min(gs.ncx - 1, (int)(cx0 / gs.wxS_d));
       ry = min(gs.ncell - 1, (int)(cy0 / gs.wS_d));
       rz = min(gs.ncell - 1, (int)(cz0 / gs.wS_d));
-      X = (float)((double)tp.x + (double)mx * gt.wS_d + (cx0 - ((double)rx + 0.5) * gs.wS_d));
+      X = (float)((double)tp.x + (double)mx * gt.wxS_d + (cx0 - ((double)rx + 0.5) * gs.wxS_d));
       Y = (float)((double)tp.y + (double)my * gt.wS_d + (cy0 - ((double)ry + 0.5) * gs.wS_d));
       Z = (float)((double)tp.z + (double)mz * gt.wS_d + (cz0 - ((double)rz + 0.5) * gs.wS_d));
     }
-    // bounding sphere of the chunk
-    float lo_x = X, hi_x = X, lo_y = Y, hi_y = Y, lo_z = Z, hi_z = Z;
+    // bounding box of the chunk (lanes >= nvalid mirror target 0)
+    Box b = {X, X, Y, Y, Z, Z};
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) {
-      lo_x = fminf(lo_x, __shfl_xor_sync(0xffffffffu, lo_x, o));
-      hi_x = fmaxf(hi_x, __shfl_xor_sync(0xffffffffu, hi_x, o));
-      lo_y = fminf(lo_y, __shfl_xor_sync(0xffffffffu, lo_y, o));
-      hi_y = fmaxf(hi_y, __shfl_xor_sync(0xffffffffu, hi_y, o));
-      lo_z = fminf(lo_z, __shfl_xor_sync(0xffffffffu, lo_z, o));
-      hi_z = fmaxf(hi_z, __shfl_xor_sync(0xffffffffu, hi_z, o));
+      b.lo_x = fminf(b.lo_x, __shfl_xor_sync(0xffffffffu, b.lo_x, o));
+      b.hi_x = fmaxf(b.hi_x, __shfl_xor_sync(0xffffffffu, b.hi_x, o));
+      b.lo_y = fminf(b.lo_y, __shfl_xor_sync(0xffffffffu, b.lo_y, o));
+      b.hi_y = fmaxf(b.hi_y, __shfl_xor_sync(0xffffffffu, b.hi_y, o));
+      b.lo_z = fminf(b.lo_z, __shfl_xor_sync(0xffffffffu, b.lo_z, o));
+      b.hi_z = fmaxf(b.hi_z, __shfl_xor_sync(0xffffffffu, b.hi_z, o));
     }
-    Frame f;
-    f.cX = 0.5f * (lo_x + hi_x);
-    f.cY = 0.5f * (lo_y + hi_y);
-    f.cZ = 0.5f * (lo_z + hi_z);
-    f.wS = gs.wS;
-    float rho2 = (X - f.cX) * (X - f.cX) + (Y - f.cY) * (Y - f.cY) + (Z - f.cZ) * (Z - f.cZ);
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) rho2 = fmaxf(rho2, __shfl_xor_sync(0xffffffffu, rho2, o));
-    const float R = A.rcS + sqrtf(rho2) * 1.0001f + 1.0e-4f;
-    f.R2 = R * R;
-
     Targets t;
 #pragma unroll
     for (int p = 0; p < NP; ++p) {
@@ -415,9 +378,9 @@ __global__ void __launch_bounds__(WARPS * 32, 3) k2_chunk_kernel(const ChunkArgs
     k.a2 = dup(c.a);
     k.B2 = dup(like ? c.B_like : c.B_unlike);
     if (chunk_p && sp == 0)
-      source_pass<true, CUT, ENERGY, STATS>(A, c, sh, lane, gs, rx, ry, rz, f, R, t, acc, k, st);
+      source_pass<true, CUT, ENERGY, STATS>(A, c, sh, lane, gs, rx, ry, rz, b, t, acc, k, st);
     else
-      source_pass<false, CUT, ENERGY, STATS>(A, c, sh, lane, gs, rx, ry, rz, f, R, t, acc, k, st);
+      source_pass<false, CUT, ENERGY, STATS>(A, c, sh, lane, gs, rx, ry, rz, b, t, acc, k, st);
   }
 
   // ---- combine the lanes' FP32 partials in FP64: quantity index = 4 * target + {fx, fy, fz, e} ------------
@@ -452,17 +415,26 @@ __global__ void __launch_bounds__(WARPS * 32, 3) k2_chunk_kernel(const ChunkArgs
 int k2_chunk_forces(Sim* s, bool with_energy, bool stats) {
   const PairConsts c = make_pair_consts(s->prm);
   const double sigma = sqrt(1.4426950408889634074 / (2.0 * s->prm.Lambda));
+  if (s->N >= (1ll << 26)) {
+    set_error("the chunk pair kernel packs slot numbers in 26 bits: N must be below 2^26");
+    return PASTA_EINVAL;
+  }
   ChunkArgs A;
   A.N = (int32_t)s->N;
   A.Np = (int32_t)s->Np;
   A.n_chunks_p = (int32_t)((s->Np + T - 1) / T);
   A.n_chunks = A.n_chunks_p + (int32_t)((s->N - s->Np + T - 1) / T);
   for (int sp = 0; sp < 2; ++sp) {
-    A.g[sp].ncell = s->grid_sp[sp].ncell;
+    const Grid& g = s->grid_sp[sp];
+    A.g[sp].ncell = g.ncell;
+    A.g[sp].ncx = g.ncx;
     A.g[sp].base = (int32_t)s->bin_base[sp];
-    A.g[sp].wS_d = sigma * s->grid_sp[sp].w;
+    A.g[sp].wS_d = sigma * g.w;
+    A.g[sp].wxS_d = sigma * g.wx;
     A.g[sp].wS = (float)A.g[sp].wS_d;
     A.g[sp].inv_wS = (float)(1.0 / A.g[sp].wS_d);
+    A.g[sp].wxS = (float)A.g[sp].wxS_d;
+    A.g[sp].inv_wxS = (float)(1.0 / A.g[sp].wxS_d);
   }
   A.rcS = (float)(sigma * s->prm.r_c);
   A.pos4 = s->pos4.as<float4>();

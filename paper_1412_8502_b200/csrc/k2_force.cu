@@ -98,7 +98,7 @@ __global__ void __launch_bounds__(128) k2_v0_kernel(V0Args A, PairConsts c) {
   if (t >= A.N) return;
   const float4 pi = A.pos4[t];
   const int ci = A.cxyz[t];
-  const int cix = ci & 1023, ciy = (ci >> 10) & 1023, ciz = (ci >> 20) & 1023;
+  const int cix = PASTA_CX(ci), ciy = PASTA_CY(ci), ciz = PASTA_CZ(ci);
   const bool ip = t < A.Np;
   double Fx = 0.0, Fy = 0.0, Fz = 0.0, E = 0.0;
   unsigned long long count = 0;
@@ -146,9 +146,9 @@ __global__ void __launch_bounds__(128) k2_v0_kernel(V0Args A, PairConsts c) {
         if (j != t) {
           const float4 pj = A.pos4[j];
           const int cj = A.cxyz[j];
-          float ddx = fmaf((float)(cix - (cj & 1023)), A.wS, pi.x - pj.x);
-          float ddy = fmaf((float)(ciy - ((cj >> 10) & 1023)), A.wS, pi.y - pj.y);
-          float ddz = fmaf((float)(ciz - ((cj >> 20) & 1023)), A.wS, pi.z - pj.z);
+          float ddx = fmaf((float)(cix - PASTA_CX(cj)), A.wS, pi.x - pj.x);
+          float ddy = fmaf((float)(ciy - PASTA_CY(cj)), A.wS, pi.y - pj.y);
+          float ddz = fmaf((float)(ciz - PASTA_CZ(cj)), A.wS, pi.z - pj.z);
           ddx -= A.LS * rintf(ddx * A.inv_LS);  // nearest periodic image
           ddy -= A.LS * rintf(ddy * A.inv_LS);
           ddz -= A.LS * rintf(ddz * A.inv_LS);

@@ -151,6 +151,7 @@ int pasta_params_default(pasta_params* p) {
   p->force_variant = 0;
   p->energy_every_step = 1;
   p->auto_grid = 1;
+  p->x_subdiv = 0;
   return PASTA_OK;
 }
 

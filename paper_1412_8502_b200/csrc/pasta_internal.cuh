@@ -39,12 +39,20 @@ void buffer_release(Sim* s, Buffer* b);
 
 // ---- grid of the force cell list (host-side description, recomputed whenever L changes) ------------
 struct Grid {
-  int32_t ncell = 1;   // cells per side
-  int64_t nc3 = 1;     // ncell^3
+  int32_t ncell = 1;   // cells per side in y and z (and in x when xsub == 1)
+  int32_t xsub = 1;    // the force grids slice every cell into xsub thin cells along x
+  int32_t ncx = 1;     // ncell * xsub
+  int64_t nc3 = 1;     // number of cells: ncell^2 * ncx
   double inv_w = 1.0;  // ncell / L  (FP64 division on the host, D14)
   double w = 1.0;      // L / ncell
+  double inv_wx = 1.0; // ncx / L
+  double wx = 1.0;     // L / ncx
 };
-Grid make_grid(double L, double r_c, int32_t k);
+Grid make_grid(double L, double r_c, int32_t k, int32_t xsub = 1);
+// packed cell coordinates of a sorted slot: cx (12 bits) | cy << 12 (10 bits) | cz << 22 (10 bits)
+#define PASTA_CX(c) ((c) & 4095)
+#define PASTA_CY(c) (((c) >> 12) & 1023)
+#define PASTA_CZ(c) (((c) >> 22) & 1023)
 
 // Constants of the FP32 pair arithmetic, derived on the host in FP64 (k2_force.cu explains them).
 struct PairConsts {
