@@ -298,7 +298,7 @@ __device__ __forceinline__ int min_image_cells(int m, int nc) {
 }
 
 template <bool CUT, bool ENERGY, bool STATS>
-__global__ void __launch_bounds__(WARPS * 32, 3) k2_chunk_kernel(const ChunkArgs A, const PairConsts c) {
+__global__ void __launch_bounds__(WARPS * 32, 4) k2_chunk_kernel(const ChunkArgs A, const PairConsts c) {
   __shared__ WarpShared shared[WARPS];
   const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
   const int chunk = blockIdx.x * WARPS + wib;
