@@ -31,8 +31,8 @@ constexpr int T = 8;            // targets per chunk
 constexpr int NP = T / 2;       // packed target pairs
 constexpr int WARPS = 4;        // warps (= chunks) per block
 constexpr int DEPTH = 4;        // cp.async stages per warp
-constexpr int TILE_CAP = 512;   // tile descriptors per warp
-constexpr int EMIT_MAX = 8;     // tiles one lane may add per emission round (32 * 8 = half the table)
+constexpr int SEG_CAP = 224;    // segment records per warp (7 rounds of 32 rows)
+constexpr float XOFF_IDLE = 1.0e12f;  // cell offset given to idle lanes: puts their source ~1e11 away
 constexpr float FAR = 1.0e10f;  // coordinate of padding sources/targets: exp2(-FAR^2) == 0, 0 * FAR == 0
 
 __device__ __forceinline__ float ex2_approx(float x) {
@@ -79,14 +79,19 @@ struct ChunkArgs {
   unsigned long long* stats;  // [0] sources streamed, [1] tiles, [2] pair evaluations (STATS only)
 };
 
-// <= 32 consecutive slots of one periodic image of a row: x = (start << 6) | (count - 1); y = xoff (add to
-// pos4.w, the thin-cell index, to get the cell offset from the frame's reference cell); z, w = the row's
-// y and z offsets from the reference cell centre, already multiplied by the cell width.
-typedef float4 Tile;
-
+// Shared memory of one warp.  The sources of a pass form one STREAM: the concatenation of its segments
+// (runs of consecutive sorted slots, one periodic image of part of a row of cells each).  Tile j of the
+// stream is positions [32 j, 32 j + 32): always full except the last one, whatever the segment lengths.
+//   seg[k]  = { int bits: first slot - stream position of the segment's start, xoff, yoff, zoff }
+//             xoff: add to pos4.w (thin-cell index) to get the cell offset from the frame's reference
+//             cell; yoff, zoff: the row's offsets from the reference cell centre, times the cell width
+//   cum[k]  = stream position at which segment k starts (cum[nseg] = stream length, then +infinity)
+//   stage   = raw pos4 of the tile's sources (cp.async), meta = the lane's {xoff, yoff, zoff} for it
 struct WarpShared {
   float4 stage[DEPTH][32];
-  Tile tile[TILE_CAP];
+  float4 meta[DEPTH][32];
+  float4 seg[SEG_CAP + 1];
+  int cum[SEG_CAP + 1 + 32];
 };
 
 // Targets and accumulators of one warp.  Targets are replicated in all lanes; accumulators hold this
@@ -146,48 +151,65 @@ __device__ __forceinline__ int floor_div(int a, int b) {  // b > 0
   return (a % b < 0) ? q - 1 : q;
 }
 
-// Stream the listed tiles through the cp.async ring and evaluate every source against the 8 targets.
+// Predicated 16-byte cp.async (no copy, and no zero fill, when pred is false).
+__device__ __forceinline__ void cp_async16_if(void* smem_dst, const void* gmem_src, bool pred) {
+  const unsigned d = (unsigned)__cvta_generic_to_shared(smem_dst);
+  asm volatile(
+      "{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %2, 0;\n\t@p cp.async.ca.shared.global [%0], [%1], 16;\n\t}\n" ::"r"(d),
+      "l"(gmem_src), "r"((int)pred)
+      : "memory");
+}
+
+// Stream the listed segments through the cp.async ring, 32 stream positions at a time, and evaluate
+// every source against the 8 targets.  Which segment a lane's position falls in is found per tile with
+// one warp OR-reduction over the segment boundaries inside the tile.
 template <bool COUL, bool CUT, bool ENERGY, bool STATS>
-__device__ __forceinline__ void run_tiles(const ChunkArgs& A, const PairConsts& c, WarpShared& sh, const int lane,
-                                          const int ntile, const float wxS, const Targets& t, Accum& acc,
-                                          const PassConsts& k, unsigned long long* st) {
-  if (ntile == 0) return;
+__device__ __forceinline__ void run_stream(const ChunkArgs& A, const PairConsts& c, WarpShared& sh, const int lane,
+                                           const int nseg, const int total, const float wxS, const Targets& t,
+                                           Accum& acc, const PassConsts& k, unsigned long long* st) {
+  if (total == 0) return;
+  const int ntile = (total + 31) >> 5;
+  const unsigned le_mask = 0xffffffffu >> (31 - lane);  // lanes <= this one
+  int fs = 0;                                           // segment holding the first position of the next tile to issue
   auto issue = [&](int j, int slot) {
-    int src = 0, bytes = 0;
-    if (j < ntile) {
-      const unsigned d = __float_as_uint(sh.tile[j].x);
-      if (lane <= (int)(d & 63u)) {
-        src = (int)(d >> 6) + lane;
-        bytes = 16;
-      }
+    if (j < ntile) {  // warp-uniform
+      const int pos0 = j << 5;
+      const unsigned rel = (unsigned)(sh.cum[fs + 1 + lane] - pos0);
+      const unsigned bnd = __reduce_or_sync(0xffffffffu, rel < 32u ? (1u << rel) : 0u);
+      const int mine = fs + __popc(bnd & le_mask);
+      fs += __popc(bnd);
+      const float4 rec = sh.seg[mine];
+      const int pos = pos0 + lane;
+      cp_async16_if(&sh.stage[slot][lane], A.pos4 + (__float_as_int(rec.x) + pos), pos < total);
+      sh.meta[slot][lane] = rec;
     }
-    cp_async16(&sh.stage[slot][lane], A.pos4 + src, bytes);
     cp_async_commit();
   };
 #pragma unroll
   for (int d = 0; d < DEPTH; ++d) issue(d, d);
+  cp_async_wait<DEPTH - 1>();
+  float4 q = sh.stage[0][lane], m = sh.meta[0][lane];
   for (int i = 0; i < ntile; ++i) {
-    cp_async_wait<DEPTH - 1>();
-    const int slot = i & (DEPTH - 1);
-    const float4 q = sh.stage[slot][lane];
-    const Tile tl = sh.tile[i];
-    const int cnt1 = (int)(__float_as_uint(tl.x) & 63u);
     // source position in the frame: cell-relative coordinate + integer cell offset * cell width
     float4 s;
-    s.x = fmaf(q.w + tl.y, wxS, q.x);
-    s.y = __fadd_rn(q.y, tl.z);
-    s.z = __fadd_rn(q.z, tl.w);
+    s.x = fmaf(q.w + m.y, wxS, q.x);
+    s.y = __fadd_rn(q.y, m.z);
+    s.z = __fadd_rn(q.z, m.w);
     s.w = 0.f;
-    if (lane > cnt1) s.x = FAR;  // idle lanes of a short tile: a far-away source contributes exactly zero
-    issue(i + DEPTH, slot);      // refill the stage just read (q has been consumed above)
-    evaluate<COUL, CUT, ENERGY>(s, t, acc, k, c);
-    if (STATS && lane == 0) {
-      st[0] += (unsigned long long)(cnt1 + 1);
-      st[1] += 1ull;
-      st[2] += 32ull * T;
+    issue(i + DEPTH, i & (DEPTH - 1));  // refill the stage just consumed
+    if (i + 1 < ntile) {                // fetch the next tile's registers before the arithmetic of this one
+      cp_async_wait<DEPTH - 1>();
+      q = sh.stage[(i + 1) & (DEPTH - 1)][lane];
+      m = sh.meta[(i + 1) & (DEPTH - 1)][lane];
     }
+    evaluate<COUL, CUT, ENERGY>(s, t, acc, k, c);
   }
   cp_async_wait<0>();
+  if (STATS && lane == 0) {
+    st[0] += (unsigned long long)total;
+    st[1] += (unsigned long long)ntile;
+    st[2] += 32ull * T * (unsigned long long)ntile;
+  }
 }
 
 // Bounding box of the chunk in the frame of a pass.
@@ -195,7 +217,7 @@ struct Box {
   float lo_x, hi_x, lo_y, hi_y, lo_z, hi_z;
 };
 
-// One pass of a chunk over one source species: list the tiles, stream them.
+// One pass of a chunk over one source species: list the segments, stream them.
 template <bool COUL, bool CUT, bool ENERGY, bool STATS>
 __device__ __forceinline__ void source_pass(const ChunkArgs& A, const PairConsts& c, WarpShared& sh, const int lane,
                                             const SpeciesGrid& gs, const int rx, const int ry, const int rz,
@@ -209,7 +231,20 @@ __device__ __forceinline__ void source_pass(const ChunkArgs& A, const PairConsts
   const int mz_lo = (int)floorf((b.lo_z - rc) * gs.inv_wS + 0.5f), mz_hi = (int)floorf((b.hi_z + rc) * gs.inv_wS + 0.5f);
   const int ny = my_hi - my_lo + 1, nrows = ny * (mz_hi - mz_lo + 1);
   const int nc = gs.ncell, ncx = gs.ncx;
-  int ntile = 0;
+  const unsigned lt_mask = (1u << lane) - 1u;
+  int nseg_list = 0, total = 0;
+
+  // close the list (dummy record for idle lanes, +infinity boundaries) and stream it
+  auto flush = [&]() {
+    if (lane == 0) sh.seg[nseg_list] = make_float4(0.f, XOFF_IDLE, 0.f, 0.f);
+    sh.cum[nseg_list + lane] = lane == 0 ? total : 0x3fffffff;
+    if (lane == 0) sh.cum[nseg_list + 32] = 0x3fffffff;
+    __syncwarp();
+    run_stream<COUL, CUT, ENERGY, STATS>(A, c, sh, lane, nseg_list, total, gs.wxS, t, acc, k, st);
+    nseg_list = 0;
+    total = 0;
+    __syncwarp();
+  };
 
   for (int rbase = 0; rbase < nrows; rbase += 32) {
     const int r = rbase + lane;
@@ -236,6 +271,7 @@ __device__ __forceinline__ void source_pass(const ChunkArgs& A, const PairConsts
       }
     }
     for (int round = 0; __any_sync(0xffffffffu, round < nseg); ++round) {
+      if (nseg_list + 32 > SEG_CAP) flush();  // (warp-uniform) list full: stream what is there
       int start = 0, len = 0;
       float xoff = 0.f;
       if (round < nseg) {
@@ -245,35 +281,24 @@ __device__ __forceinline__ void source_pass(const ChunkArgs& A, const PairConsts
         len = __ldg(A.bin_start + rowbase + a_hi + 1) - start;
         xoff = (float)(qb - rx);
       }
-      // emit the segment's tiles, at most EMIT_MAX per lane and round trip, so the table never overflows
-      while (__any_sync(0xffffffffu, len > 0)) {
-        if (ntile + 32 * EMIT_MAX > TILE_CAP) {  // (warp-uniform) table nearly full: stream what is there
-          __syncwarp();
-          run_tiles<COUL, CUT, ENERGY, STATS>(A, c, sh, lane, ntile, gs.wxS, t, acc, k, st);
-          ntile = 0;
-          __syncwarp();
-        }
-        const int mine = min((len + 31) >> 5, EMIT_MAX);
-        int incl = mine;
+      // append the non-empty segments in lane order; stream positions by an inclusive scan of the lengths
+      int incl = len;
 #pragma unroll
-        for (int o = 1; o < 32; o <<= 1) {
-          const int v = __shfl_up_sync(0xffffffffu, incl, o);
-          if (lane >= o) incl += v;
-        }
-        int at = ntile + incl - mine;
-        for (int m = 0; m < mine; ++m) {
-          const int cnt = min(len, 32);
-          sh.tile[at++] = make_float4(__uint_as_float(((unsigned)start << 6) | (unsigned)(cnt - 1)), xoff, yoff, zoff);
-          start += cnt;
-          len -= cnt;
-        }
-        ntile += __shfl_sync(0xffffffffu, incl, 31);
+      for (int o = 1; o < 32; o <<= 1) {
+        const int v = __shfl_up_sync(0xffffffffu, incl, o);
+        if (lane >= o) incl += v;
       }
+      const unsigned has = __ballot_sync(0xffffffffu, len > 0);
+      if (len > 0) {
+        const int at = nseg_list + __popc(has & lt_mask), begin = total + incl - len;
+        sh.seg[at] = make_float4(__int_as_float(start - begin), xoff, yoff, zoff);
+        sh.cum[at] = begin;
+      }
+      nseg_list += __popc(has);
+      total += __shfl_sync(0xffffffffu, incl, 31);
     }
   }
-  __syncwarp();
-  run_tiles<COUL, CUT, ENERGY, STATS>(A, c, sh, lane, ntile, gs.wxS, t, acc, k, st);
-  __syncwarp();
+  flush();
 }
 
 // Sum v over the warp for 32 different quantities at once: on entry lane l holds its partial of quantity
@@ -304,6 +329,8 @@ __global__ void __launch_bounds__(WARPS * 32, 4) k2_chunk_kernel(const ChunkArgs
   const int chunk = blockIdx.x * WARPS + wib;
   if (chunk >= A.n_chunks) return;
   WarpShared& sh = shared[wib];
+#pragma unroll
+  for (int d = 0; d < DEPTH; ++d) sh.stage[d][lane] = make_float4(0.f, 0.f, 0.f, 0.f);  // idle lanes read it
 
   const bool chunk_p = chunk < A.n_chunks_p;
   const int st_sp = chunk_p ? 0 : 1;
