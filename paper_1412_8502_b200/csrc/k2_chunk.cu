@@ -29,7 +29,16 @@ namespace {
 
 constexpr int T = 8;            // targets per chunk
 constexpr int NP = T / 2;       // packed target pairs
-constexpr int WARPS = 4;        // warps (= chunks) per block
+#ifndef K2_MINB
+#define K2_MINB 4
+#endif
+#ifndef K2_UNIFORM
+#define K2_UNIFORM 1
+#endif
+#ifndef K2_WARPS
+#define K2_WARPS 4
+#endif
+constexpr int WARPS = K2_WARPS;  // warps (= chunks) per block
 constexpr int DEPTH = 4;        // cp.async stages per warp
 constexpr int SEG_CAP = 224;    // segment records per warp (7 rounds of 32 rows)
 constexpr float XOFF_IDLE = 1.0e12f;  // cell offset given to idle lanes: puts their source ~1e11 away
@@ -44,6 +53,10 @@ __device__ __forceinline__ float rsqrt_approx(float x) {
   float y;
   asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
   return y;
+}
+// Broadcast of lane `src`'s value through REDUX.OR: the result is provably warp-uniform (a uniform register).
+__device__ __forceinline__ float bcast_uniform(float v, int lane, int src) {
+  return __int_as_float(__reduce_or_sync(0xffffffffu, lane == src ? __float_as_int(v) : 0));
 }
 __device__ __forceinline__ float2 dup(float a) { return make_float2(a, a); }
 __device__ __forceinline__ float2 neg2(float2 a) { return make_float2(-a.x, -a.y); }
@@ -88,8 +101,6 @@ struct ChunkArgs {
 //   cum[k]  = stream position at which segment k starts (cum[nseg] = stream length, then +infinity)
 //   stage   = raw pos4 of the tile's sources (cp.async), meta = the lane's {xoff, yoff, zoff} for it
 struct WarpShared {
-  float4 stage[DEPTH][32];
-  float4 meta[DEPTH][32];
   float4 seg[SEG_CAP + 1];
   int cum[SEG_CAP + 1 + 32];
 };
@@ -109,38 +120,48 @@ struct PassConsts {
 template <bool COUL, bool CUT, bool ENERGY>
 __device__ __forceinline__ void evaluate(const float4 s, const Targets& t, Accum& acc, const PassConsts& k,
                                          const PairConsts& c) {
+  // phase 1: displacements and -r'^2 of all 8 pairs; phase 2: the 8 exponentials back to back on the MUFU;
+  // phase 3: polynomials and accumulation.  (Written in phases so that the MUFU latency of one pair is
+  // covered by the arithmetic of the others.)
+  float2 dx[NP], dy[NP], dz[NP], nr2[NP], u[NP];
 #pragma unroll
   for (int p = 0; p < NP; ++p) {
-    const float2 dx = __fadd2_rn(dup(s.x), t.ntx[p]);
-    const float2 dy = __fadd2_rn(dup(s.y), t.nty[p]);
-    const float2 dz = __fadd2_rn(dup(s.z), t.ntz[p]);
+    dx[p] = __fadd2_rn(dup(s.x), t.ntx[p]);
+    dy[p] = __fadd2_rn(dup(s.y), t.nty[p]);
+    dz[p] = __fadd2_rn(dup(s.z), t.ntz[p]);
     // minus r'^2, accumulated with negated operands (free on FFMA2) because MUFU.EX2 takes no negation
-    float2 nr2 = __fmul2_rn(neg2(dx), dx);
-    nr2 = __ffma2_rn(neg2(dy), dy, nr2);
-    nr2 = __ffma2_rn(neg2(dz), dz, nr2);
-    float2 u = make_float2(ex2_approx(nr2.x), ex2_approx(nr2.y));
+    nr2[p] = __fmul2_rn(neg2(dx[p]), dx[p]);
+    nr2[p] = __ffma2_rn(neg2(dy[p]), dy[p], nr2[p]);
+    nr2[p] = __ffma2_rn(neg2(dz[p]), dz[p], nr2[p]);
+  }
+#pragma unroll
+  for (int p = 0; p < NP; ++p) {
+    u[p] = make_float2(ex2_approx(nr2[p].x), ex2_approx(nr2[p].y));
     if (CUT) {
-      u.x = nr2.x > -c.rc2s ? u.x : 0.f;
-      u.y = nr2.y > -c.rc2s ? u.y : 0.f;
+      u[p].x = nr2[p].x > -c.rc2s ? u[p].x : 0.f;
+      u[p].y = nr2[p].y > -c.rc2s ? u[p].y : 0.f;
     }
-    float2 g = __fmul2_rn(u, __ffma2_rn(k.g2a, u, k.gB));
+  }
+#pragma unroll
+  for (int p = 0; p < NP; ++p) {
+    float2 g = __fmul2_rn(u[p], __ffma2_rn(k.g2a, u[p], k.gB));
     float2 V;
-    if (ENERGY) V = __fmul2_rn(u, __ffma2_rn(k.a2, u, k.B2));
+    if (ENERGY) V = __fmul2_rn(u[p], __ffma2_rn(k.a2, u[p], k.B2));
     if (COUL) {
       // screened Coulomb, cut at r_c, skipped at r = 0 (the self pair and coincident protons, D2):
       // 1/r' := 0 for excluded pairs, which zeroes every Coulomb factor without creating inf * 0
-      const bool in0 = nr2.x > -c.rc2s && nr2.x < 0.f, in1 = nr2.y > -c.rc2s && nr2.y < 0.f;
-      const float2 rinv = make_float2(in0 ? rsqrt_approx(-nr2.x) : 0.f, in1 ? rsqrt_approx(-nr2.y) : 0.f);
-      const float2 nr = __fmul2_rn(nr2, rinv);  // -r'
+      const bool in0 = nr2[p].x > -c.rc2s && nr2[p].x < 0.f, in1 = nr2[p].y > -c.rc2s && nr2[p].y < 0.f;
+      const float2 rinv = make_float2(in0 ? rsqrt_approx(-nr2[p].x) : 0.f, in1 ? rsqrt_approx(-nr2[p].y) : 0.f);
+      const float2 nr = __fmul2_rn(nr2[p], rinv);  // -r'
       const float2 ex = make_float2(ex2_approx(c.kappa * nr.x), ex2_approx(c.kappa * nr.y));
       const float2 tq = __fmul2_rn(ex, rinv);
       if (ENERGY) V = __ffma2_rn(dup(c.alpha_s), tq, V);
       const float2 q = __fmul2_rn(__fadd2_rn(rinv, dup(c.inv_lam_s)), rinv);
       g = __ffma2_rn(__fmul2_rn(dup(c.alpha_s2), tq), q, g);
     }
-    acc.fx[p] = __ffma2_rn(g, dx, acc.fx[p]);
-    acc.fy[p] = __ffma2_rn(g, dy, acc.fy[p]);
-    acc.fz[p] = __ffma2_rn(g, dz, acc.fz[p]);
+    acc.fx[p] = __ffma2_rn(g, dx[p], acc.fx[p]);
+    acc.fy[p] = __ffma2_rn(g, dy[p], acc.fy[p]);
+    acc.fz[p] = __ffma2_rn(g, dz[p], acc.fz[p]);
     if (ENERGY) acc.e[p] = __fadd2_rn(acc.e[p], V);
   }
 }
@@ -151,64 +172,69 @@ __device__ __forceinline__ int floor_div(int a, int b) {  // b > 0
   return (a % b < 0) ? q - 1 : q;
 }
 
-// Predicated 16-byte cp.async (no copy, and no zero fill, when pred is false).
-__device__ __forceinline__ void cp_async16_if(void* smem_dst, const void* gmem_src, bool pred) {
-  const unsigned d = (unsigned)__cvta_generic_to_shared(smem_dst);
-  asm volatile(
-      "{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %2, 0;\n\t@p cp.async.ca.shared.global [%0], [%1], 16;\n\t}\n" ::"r"(d),
-      "l"(gmem_src), "r"((int)pred)
-      : "memory");
+// Per-lane cursor into the segment list of a pass: the segment holding the lane's current stream position.
+struct Cursor {
+  int cur;     // segment index
+  int end;     // stream position at which segment `cur` ends
+  float4 rec;  // its record
+};
+
+// Raw source of stream position `pos` for this lane (zeros past the end of the stream) and the record of the
+// segment it belongs to.  A lane's positions grow by 32 per tile, so the cursor only ever moves forward.
+__device__ __forceinline__ void fetch(const ChunkArgs& A, const WarpShared& sh, Cursor& cu, const int pos,
+                                      const int total, float4& q, float4& m) {
+  if (pos >= cu.end) {
+    do {
+      ++cu.cur;
+      cu.end = sh.cum[cu.cur + 1];
+    } while (pos >= cu.end);
+    cu.rec = sh.seg[cu.cur];
+  }
+  m = cu.rec;
+  q = make_float4(0.f, 0.f, 0.f, 0.f);
+  if (pos < total) q = __ldg(A.pos4 + (__float_as_int(cu.rec.x) + pos));
 }
 
-// Stream the listed segments through the cp.async ring, 32 stream positions at a time, and evaluate
-// every source against the 8 targets.  Which segment a lane's position falls in is found per tile with
-// one warp OR-reduction over the segment boundaries inside the tile.
+// source position in the frame: cell-relative coordinate + integer cell offset * cell width
+__device__ __forceinline__ float4 to_frame(const float4 q, const float4 m, const float wxS) {
+  float4 s;
+  s.x = fmaf(q.w + m.y, wxS, q.x);
+  s.y = __fadd_rn(q.y, m.z);
+  s.z = __fadd_rn(q.z, m.w);
+  s.w = 0.f;
+  return s;
+}
+
+// Stream the listed segments, 32 stream positions at a time, and evaluate every source against the 8
+// targets.  Sources are fetched straight into registers two tiles ahead (the positions are L2-resident);
+// the loop handles two tiles per trip so that the double buffer needs no register moves.  An odd tail is
+// padded with one tile of idle lanes, which contribute exact zeros.
 template <bool COUL, bool CUT, bool ENERGY, bool STATS>
 __device__ __forceinline__ void run_stream(const ChunkArgs& A, const PairConsts& c, WarpShared& sh, const int lane,
                                            const int nseg, const int total, const float wxS, const Targets& t,
                                            Accum& acc, const PassConsts& k, unsigned long long* st) {
   if (total == 0) return;
   const int ntile = (total + 31) >> 5;
-  const unsigned le_mask = 0xffffffffu >> (31 - lane);  // lanes <= this one
-  int fs = 0;                                           // segment holding the first position of the next tile to issue
-  auto issue = [&](int j, int slot) {
-    if (j < ntile) {  // warp-uniform
-      const int pos0 = j << 5;
-      const unsigned rel = (unsigned)(sh.cum[fs + 1 + lane] - pos0);
-      const unsigned bnd = __reduce_or_sync(0xffffffffu, rel < 32u ? (1u << rel) : 0u);
-      const int mine = fs + __popc(bnd & le_mask);
-      fs += __popc(bnd);
-      const float4 rec = sh.seg[mine];
-      const int pos = pos0 + lane;
-      cp_async16_if(&sh.stage[slot][lane], A.pos4 + (__float_as_int(rec.x) + pos), pos < total);
-      sh.meta[slot][lane] = rec;
-    }
-    cp_async_commit();
-  };
-#pragma unroll
-  for (int d = 0; d < DEPTH; ++d) issue(d, d);
-  cp_async_wait<DEPTH - 1>();
-  float4 q = sh.stage[0][lane], m = sh.meta[0][lane];
-  for (int i = 0; i < ntile; ++i) {
-    // source position in the frame: cell-relative coordinate + integer cell offset * cell width
-    float4 s;
-    s.x = fmaf(q.w + m.y, wxS, q.x);
-    s.y = __fadd_rn(q.y, m.z);
-    s.z = __fadd_rn(q.z, m.w);
-    s.w = 0.f;
-    issue(i + DEPTH, i & (DEPTH - 1));  // refill the stage just consumed
-    if (i + 1 < ntile) {                // fetch the next tile's registers before the arithmetic of this one
-      cp_async_wait<DEPTH - 1>();
-      q = sh.stage[(i + 1) & (DEPTH - 1)][lane];
-      m = sh.meta[(i + 1) & (DEPTH - 1)][lane];
-    }
-    evaluate<COUL, CUT, ENERGY>(s, t, acc, k, c);
+  Cursor cu;
+  cu.cur = 0;
+  cu.end = sh.cum[1];
+  cu.rec = sh.seg[0];
+  float4 qa, ma, qb, mb;
+  fetch(A, sh, cu, lane, total, qa, ma);
+  fetch(A, sh, cu, 32 + lane, total, qb, mb);
+#pragma unroll 1
+  for (int i = 0; i < ntile; i += 2) {
+    const float4 sa = to_frame(qa, ma, wxS);
+    fetch(A, sh, cu, ((i + 2) << 5) + lane, total, qa, ma);
+    evaluate<COUL, CUT, ENERGY>(sa, t, acc, k, c);
+    const float4 sb = to_frame(qb, mb, wxS);
+    fetch(A, sh, cu, ((i + 3) << 5) + lane, total, qb, mb);
+    evaluate<COUL, CUT, ENERGY>(sb, t, acc, k, c);
   }
-  cp_async_wait<0>();
   if (STATS && lane == 0) {
     st[0] += (unsigned long long)total;
-    st[1] += (unsigned long long)ntile;
-    st[2] += 32ull * T * (unsigned long long)ntile;
+    st[1] += (unsigned long long)((ntile + 1) & ~1);
+    st[2] += 32ull * T * (unsigned long long)((ntile + 1) & ~1);
   }
 }
 
@@ -323,14 +349,19 @@ __device__ __forceinline__ int min_image_cells(int m, int nc) {
 }
 
 template <bool CUT, bool ENERGY, bool STATS>
-__global__ void __launch_bounds__(WARPS * 32, 4) k2_chunk_kernel(const ChunkArgs A, const PairConsts c) {
+__global__ void __launch_bounds__(WARPS * 32, K2_MINB) k2_chunk_kernel(const ChunkArgs A, const PairConsts c) {
   __shared__ WarpShared shared[WARPS];
-  const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
+  const int lane = threadIdx.x & 31;
+#if K2_UNIFORM
+  // warp-uniform values are produced by REDUX so that the compiler can prove them uniform and keep them
+  // (and everything derived from them) in uniform registers, off the vector register file
+  const int wib = __reduce_or_sync(0xffffffffu, (int)(threadIdx.x >> 5));
+#else
+  const int wib = threadIdx.x >> 5;
+#endif
   const int chunk = blockIdx.x * WARPS + wib;
   if (chunk >= A.n_chunks) return;
   WarpShared& sh = shared[wib];
-#pragma unroll
-  for (int d = 0; d < DEPTH; ++d) sh.stage[d][lane] = make_float4(0.f, 0.f, 0.f, 0.f);  // idle lanes read it
 
   const bool chunk_p = chunk < A.n_chunks_p;
   const int st_sp = chunk_p ? 0 : 1;
@@ -390,6 +421,13 @@ __global__ void __launch_bounds__(WARPS * 32, 4) k2_chunk_kernel(const ChunkArgs
     Targets t;
 #pragma unroll
     for (int p = 0; p < NP; ++p) {
+#if K2_UNIFORM
+      // lane j < 8 contributes minus its coordinate (FAR if it holds no valid target), every other lane 0
+      const float nX = lane < nvalid ? -X : FAR, nY = lane < nvalid ? -Y : FAR, nZ = lane < nvalid ? -Z : FAR;
+      t.ntx[p] = make_float2(bcast_uniform(nX, lane, 2 * p), bcast_uniform(nX, lane, 2 * p + 1));
+      t.nty[p] = make_float2(bcast_uniform(nY, lane, 2 * p), bcast_uniform(nY, lane, 2 * p + 1));
+      t.ntz[p] = make_float2(bcast_uniform(nZ, lane, 2 * p), bcast_uniform(nZ, lane, 2 * p + 1));
+#else
       const float x0 = __shfl_sync(0xffffffffu, X, 2 * p), x1 = __shfl_sync(0xffffffffu, X, 2 * p + 1);
       const float y0 = __shfl_sync(0xffffffffu, Y, 2 * p), y1 = __shfl_sync(0xffffffffu, Y, 2 * p + 1);
       const float z0 = __shfl_sync(0xffffffffu, Z, 2 * p), z1 = __shfl_sync(0xffffffffu, Z, 2 * p + 1);
@@ -397,6 +435,7 @@ __global__ void __launch_bounds__(WARPS * 32, 4) k2_chunk_kernel(const ChunkArgs
       t.ntx[p] = make_float2(v0 ? -x0 : FAR, v1 ? -x1 : FAR);
       t.nty[p] = make_float2(v0 ? -y0 : FAR, v1 ? -y1 : FAR);
       t.ntz[p] = make_float2(v0 ? -z0 : FAR, v1 ? -z1 : FAR);
+#endif
     }
     const bool like = sp == st_sp;
     PassConsts k;
