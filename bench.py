@@ -183,6 +183,8 @@ def run_ours(args, rank, world, local_rank):
         prm.force_variant = args.variant
     if args.subdiv is not None:
         prm.cell_subdiv = args.subdiv
+    if args.stream_all:
+        prm.skip_exact_zeros = 0
     sim = pasta.Sim(N, c["Y_P"], c["density"], c["T"], params=prm, seed=1 + rank)
     flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")
 
@@ -287,6 +289,8 @@ def main():
     ap.add_argument("--config", type=int, default=4, choices=[2, 4])
     ap.add_argument("--variant", type=int, default=None, help="pasta_params.force_variant override")
     ap.add_argument("--subdiv", type=int, default=None, help="pasta_params.cell_subdiv override")
+    ap.add_argument("--stream-all", action="store_true",
+                    help="pasta_params.skip_exact_zeros = 0: stream every candidate out to r_c")
     ap.add_argument("--cpu-budget", type=float, default=15.0, help="seconds of oracle time for cpu_baseline")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()

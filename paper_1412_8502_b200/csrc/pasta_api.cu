@@ -152,6 +152,7 @@ int pasta_params_default(pasta_params* p) {
   p->energy_every_step = 1;
   p->auto_grid = 1;
   p->x_subdiv = 0;
+  p->skip_exact_zeros = 1;
   return PASTA_OK;
 }
 
