@@ -58,7 +58,7 @@ typedef struct pasta_params {
   int32_t energy_every_step;   /* 1 (default): pasta_step evaluates per-particle energies with the forces */
   int32_t auto_grid;           /* 1 (default): each species' force grid picks its own k (about 8 particles per cell);
                                   0: both use cell_subdiv.  pasta_cells always reports the cell_subdiv grid */
-  int32_t x_subdiv;            /* thin cells along x per force-grid cell (0 = library default, 4) */
+  int32_t x_subdiv;            /* thin cells along x per force-grid cell (0 = library default, 8) */
   int32_t skip_exact_zeros;    /* 1 (default): np/nn candidates beyond the distance at which exp2(-r^2 log2e/2 Lambda)
                                   underflows FP32 (14.78 fm for Lambda = 1.25) are not streamed: their terms are exactly
                                   0.0f in the kernel's arithmetic, so F and e are unchanged (D23).  0: stream to r_c */
@@ -164,6 +164,9 @@ int pasta_particle_energies(pasta_sim* sim, double* e_dev);
 /* Number of ordered in-range pairs (i != j, r_ij < r_c) of the current configuration, counted by a
  * kernel in the same FP32 arithmetic the force kernel uses: the work unit of the throughput metric. */
 int pasta_pair_count(pasta_sim* sim, int64_t* ordered_pairs_host);
+/* The same, and beside it the number of those pairs that carry a term which is not exactly 0.0f in the FP32
+ * pair arithmetic: out2_host = {in range, in range and (pp or exp2(-r^2 log2e / 2 Lambda) >= 2^-126)} (D23). */
+int pasta_pair_counts(pasta_sim* sim, int64_t* out2_host);
 
 /* Work statistics of one evaluation with the chunk pair kernel: out3_host = {sources streamed from the cell
  * rows (summed over chunks), tiles of <= 32 sources, pair evaluations executed}.  Synchronises.

@@ -65,6 +65,7 @@ SIGNATURES = {
     "pasta_energy": (C.c_int, [C.c_void_p, C.POINTER(C.c_double), C.POINTER(C.c_double)]),
     "pasta_particle_energies": (C.c_int, [C.c_void_p, C.c_void_p]),
     "pasta_pair_count": (C.c_int, [C.c_void_p, C.POINTER(C.c_int64)]),
+    "pasta_pair_counts": (C.c_int, [C.c_void_p, C.POINTER(C.c_int64)]),
     "pasta_force_stats": (C.c_int, [C.c_void_p, C.POINTER(C.c_int64)]),
     "pasta_set_timing": (C.c_int, [C.c_void_p, C.c_int32]),
     "pasta_get_timing": (C.c_int, [C.c_void_p, C.POINTER(C.c_double), C.POINTER(C.c_int64)]),
@@ -300,6 +301,12 @@ class Sim:
         n = C.c_int64()
         _check(self.lib.pasta_pair_count(self._h, C.byref(n)))
         return n.value
+
+    def pair_counts(self):
+        """(ordered in-range pairs, those with a term that is not exactly zero in FP32)."""
+        out = (C.c_int64 * 2)()
+        _check(self.lib.pasta_pair_counts(self._h, out))
+        return int(out[0]), int(out[1])
 
     def force_stats(self):
         out = (C.c_int64 * 3)()

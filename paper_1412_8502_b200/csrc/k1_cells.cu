@@ -223,7 +223,7 @@ int k1_build(Sim* s, bool uniform_grid) {
   const bool same_k = uniform || s->prm.auto_grid == 0;
   const int k0 = same_k ? s->prm.cell_subdiv : auto_subdiv(s->L, s->prm.r_c, s->Np, s->prm.cell_subdiv);
   const int k1 = same_k ? s->prm.cell_subdiv : auto_subdiv(s->L, s->prm.r_c, N - s->Np, s->prm.cell_subdiv);
-  const int xsub = uniform ? 1 : (s->prm.x_subdiv > 0 ? s->prm.x_subdiv : 4);
+  const int xsub = uniform ? 1 : (s->prm.x_subdiv > 0 ? s->prm.x_subdiv : 8);
   s->grid_sp[0] = make_grid(s->L, s->prm.r_c, k0, xsub);
   s->grid_sp[1] = make_grid(s->L, s->prm.r_c, k1, xsub);
   GridPair g;

@@ -33,7 +33,10 @@ namespace {
 #define K2_T 8
 #endif
 #ifndef K2_MINB
-#define K2_MINB 8
+#define K2_MINB 5
+#endif
+#ifndef K2_ESUM
+#define K2_ESUM 0
 #endif
 #ifndef K2_WARPS
 #define K2_WARPS 4
@@ -101,8 +104,11 @@ struct WarpShared {
 struct Targets {
   float2 ntx, nty, ntz;
 };
+// The nuclear energy of a pass is a S2 + B S1 with S1 = sum u, S2 = sum u^2 (B is constant over a pass), which
+// costs two 2-operand packed instructions per step instead of a polynomial and a 3-operand accumulate;
+// `e` holds the energy of the finished passes plus the Coulomb terms.
 struct Accum {
-  float2 fx, fy, fz, e;
+  float2 fx, fy, fz, e, s1, s2;
 };
 struct PassConsts {
   float g2a, gB, a, B;
@@ -125,8 +131,14 @@ __device__ __forceinline__ void evaluate(const float4 s, const Targets& t, Accum
     u.y = nr2.y > -c.rc2s ? u.y : 0.f;
   }
   float2 g = __fmul2_rn(u, __ffma2_rn(dup(k.g2a), u, dup(k.gB)));
-  float2 V;
-  if (ENERGY) V = __fmul2_rn(u, __ffma2_rn(dup(k.a), u, dup(k.B)));
+#if K2_ESUM
+  if (ENERGY) {
+    acc.s1 = __fadd2_rn(acc.s1, u);
+    acc.s2 = __ffma2_rn(u, u, acc.s2);
+  }
+#else
+  if (ENERGY) acc.e = __ffma2_rn(u, __ffma2_rn(dup(k.a), u, dup(k.B)), acc.e);
+#endif
   if (COUL) {
     // screened Coulomb, cut at r_c, skipped at r = 0 (the self pair and coincident protons, D2):
     // 1/r' := 0 for excluded pairs, which zeroes every Coulomb factor without creating inf * 0
@@ -135,14 +147,13 @@ __device__ __forceinline__ void evaluate(const float4 s, const Targets& t, Accum
     const float2 nr = __fmul2_rn(nr2, rinv);  // -r'
     const float2 ex = make_float2(ex2_approx(c.kappa * nr.x), ex2_approx(c.kappa * nr.y));
     const float2 tq = __fmul2_rn(ex, rinv);
-    if (ENERGY) V = __ffma2_rn(dup(c.alpha_s), tq, V);
+    if (ENERGY) acc.e = __ffma2_rn(dup(c.alpha_s), tq, acc.e);
     const float2 q = __fmul2_rn(__fadd2_rn(rinv, dup(c.inv_lam_s)), rinv);
     g = __ffma2_rn(__fmul2_rn(dup(c.alpha_s2), tq), q, g);
   }
   acc.fx = __ffma2_rn(g, dx, acc.fx);
   acc.fy = __ffma2_rn(g, dy, acc.fy);
   acc.fz = __ffma2_rn(g, dz, acc.fz);
-  if (ENERGY) acc.e = __fadd2_rn(acc.e, V);
 }
 
 __device__ __forceinline__ int floor_div(int a, int b) {  // b > 0
@@ -201,14 +212,16 @@ __device__ __forceinline__ void run_stream(const ChunkArgs& A, const PairConsts&
   cu.rec = sh.seg[0];
   float4 q, m;
   fetch(A, sh, cu, lane, total, q, m);
+  float4* const wr = &sh.tile[0][lane];
+  const float4* const rd = &sh.tile[0][ph];
 #pragma unroll 1
   for (int i = 0; i < ntile; ++i) {
-    float4* buf = sh.tile[i & 1];
-    buf[lane] = to_frame(q, m, wxS);
+    const int o = (i & 1) * 32;
+    wr[o] = to_frame(q, m, wxS);
     fetch(A, sh, cu, ((i + 1) << 5) + lane, total, q, m);
     __syncwarp();
 #pragma unroll
-    for (int j = 0; j < STEPS; ++j) evaluate<COUL, CUT, ENERGY>(buf[ph + NPH * j], t, acc, k, c);
+    for (int j = 0; j < STEPS; ++j) evaluate<COUL, CUT, ENERGY>(rd[o + NPH * j], t, acc, k, c);
   }
   __syncwarp();
   if (STATS && lane == 0) {
@@ -349,13 +362,13 @@ __global__ void __launch_bounds__(WARPS * 32, K2_MINB) k2_chunk_kernel(const Chu
   const int mz = min_image_cells(PASTA_CZ(tc) - oz, gt.ncell);
 
   Accum acc;
-  acc.fx = acc.fy = acc.fz = acc.e = make_float2(0.f, 0.f);
+  acc.fx = acc.fy = acc.fz = acc.e = acc.s1 = acc.s2 = make_float2(0.f, 0.f);
   unsigned long long st[3] = {0, 0, 0};
 
   // ---- pass 0: proton sources, pass 1: neutron sources -------------------------------------------------
-#pragma unroll 1
+#pragma unroll
   for (int sp = 0; sp < 2; ++sp) {
-    const SpeciesGrid gs = A.g[sp];
+    const SpeciesGrid& gs = A.g[sp];
     // Frame of the pass: origin = centre of the source-grid cell (rx, ry, rz) that contains the centre of
     // the chunk's origin cell.  Same grid: identical arithmetic for targets and sources (a target meets
     // itself at d == 0 exactly).  Other grid: the shift between the two cell centres is taken in FP64.
@@ -402,10 +415,14 @@ __global__ void __launch_bounds__(WARPS * 32, K2_MINB) k2_chunk_kernel(const Chu
     k.gB = like ? c.gB_like : c.gB_unlike;
     k.a = c.a;
     k.B = like ? c.B_like : c.B_unlike;
-    if (chunk_p && sp == 0)
+    if (sp == 0 && chunk_p)
       source_pass<true, CUT, ENERGY, STATS>(A, c, sh, lane, gs, rx, ry, rz, b, t, acc, k, st);
     else
       source_pass<false, CUT, ENERGY, STATS>(A, c, sh, lane, gs, rx, ry, rz, b, t, acc, k, st);
+    if (ENERGY && K2_ESUM) {  // nuclear energy of this pass: a S2 + B S1
+      acc.e = __ffma2_rn(dup(k.a), acc.s2, __ffma2_rn(dup(k.B), acc.s1, acc.e));
+      acc.s1 = acc.s2 = make_float2(0.f, 0.f);
+    }
   }
 
   // ---- combine the phases' FP32 partials in FP64 ------------------------------------------------------------

@@ -101,7 +101,7 @@ __global__ void __launch_bounds__(128) k2_v0_kernel(V0Args A, PairConsts c) {
   const int cix = PASTA_CX(ci), ciy = PASTA_CY(ci), ciz = PASTA_CZ(ci);
   const bool ip = t < A.Np;
   double Fx = 0.0, Fy = 0.0, Fz = 0.0, E = 0.0;
-  unsigned long long count = 0;
+  unsigned long long count = 0, count_nz = 0;  // in range; in range with a term that is not exactly 0 in FP32
   const bool stencil = A.ncell >= 2 * A.k + 1;
 
   for (int sj = 0; sj < 2; ++sj) {  // source species: 0 = protons, 1 = neutrons
@@ -130,6 +130,7 @@ __global__ void __launch_bounds__(128) k2_v0_kernel(V0Args A, PairConsts c) {
               if (r2 < c.rc2s) {
                 if (COUNT_ONLY) {
                   ++count;
+                  count_nz += (coul || r2 < 126.0f) ? 1 : 0;
                 } else if (coul) {
                   pair_accumulate<true, ENERGY>(ddx, ddy, ddz, r2, B, gB, c, fx, fy, fz, e);
                 } else {
@@ -156,6 +157,7 @@ __global__ void __launch_bounds__(128) k2_v0_kernel(V0Args A, PairConsts c) {
           if (r2 < c.rc2s) {
             if (COUNT_ONLY) {
               ++count;
+              count_nz += (coul || r2 < 126.0f) ? 1 : 0;
             } else if (coul) {
               pair_accumulate<true, ENERGY>(ddx, ddy, ddz, r2, B, gB, c, fx, fy, fz, e);
             } else {
@@ -172,6 +174,7 @@ __global__ void __launch_bounds__(128) k2_v0_kernel(V0Args A, PairConsts c) {
   }
   if (COUNT_ONLY) {
     if (count) atomicAdd(A.pair_counter, count);
+    if (count_nz) atomicAdd(A.pair_counter + 1, count_nz);
   } else {
     const int i = A.perm[t];
     A.F[3 * (int64_t)i + 0] = Fx;
@@ -223,18 +226,19 @@ int k2_reference_forces(Sim* s, bool with_energy) {
   return PASTA_OK;
 }
 
-int k2_pair_count(Sim* s, int64_t* ordered_pairs_host) {
+int k2_pair_count(Sim* s, int64_t* ordered_pairs_host, int64_t* nonzero_pairs_host) {
   const PairConsts c = make_pair_consts(s->prm);
   V0Args A = make_v0_args(s);
-  PASTA_CUDA_OK(cudaMemsetAsync(A.pair_counter, 0, sizeof(unsigned long long), s->stream));
+  PASTA_CUDA_OK(cudaMemsetAsync(A.pair_counter, 0, 2 * sizeof(unsigned long long), s->stream));
   const int B = 128;
   k2_v0_kernel<false, true><<<grid_for(s->N, B), B, 0, s->stream>>>(A, c);
   s->launches += 1;
   PASTA_CUDA_OK(cudaGetLastError());
-  unsigned long long h = 0;
-  PASTA_CUDA_OK(cudaMemcpyAsync(&h, A.pair_counter, sizeof(h), cudaMemcpyDeviceToHost, s->stream));
+  unsigned long long h[2] = {0, 0};
+  PASTA_CUDA_OK(cudaMemcpyAsync(h, A.pair_counter, sizeof(h), cudaMemcpyDeviceToHost, s->stream));
   PASTA_CUDA_OK(cudaStreamSynchronize(s->stream));
-  *ordered_pairs_host = (int64_t)h;
+  if (ordered_pairs_host) *ordered_pairs_host = (int64_t)h[0];
+  if (nonzero_pairs_host) *nonzero_pairs_host = (int64_t)h[1];
   return PASTA_OK;
 }
 

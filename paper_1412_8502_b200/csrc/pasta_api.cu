@@ -495,7 +495,19 @@ int pasta_pair_count(pasta_sim* sim, int64_t* ordered_pairs_host) {
   }
   PASTA_TRY(use_device(s));
   PASTA_TRY(k1_build(s, true));  // the counting kernel walks one common grid
-  return k2_pair_count(s, ordered_pairs_host);
+  return k2_pair_count(s, ordered_pairs_host, nullptr);
+}
+
+int pasta_pair_counts(pasta_sim* sim, int64_t* out2_host) {
+  Sim* s = reinterpret_cast<Sim*>(sim);
+  PASTA_TRY(check_sim(s));
+  if (!out2_host) {
+    set_error("out2_host is NULL");
+    return PASTA_EINVAL;
+  }
+  PASTA_TRY(use_device(s));
+  PASTA_TRY(k1_build(s, true));
+  return k2_pair_count(s, out2_host, out2_host + 1);
 }
 
 int pasta_force_stats(pasta_sim* sim, int64_t* out3_host) {

@@ -128,7 +128,7 @@ int k1_export_cells(Sim* s, int32_t* cell_id_dev, int32_t* cell_start_dev);
 int scan_exclusive(Sim* s, const int32_t* in, int32_t* out, int64_t n);  // out[0..n] (n+1 entries)
 // K2  k2_force.cu
 int k2_forces(Sim* s, bool with_energy);               // F, e in original order
-int k2_pair_count(Sim* s, int64_t* ordered_pairs_host);
+int k2_pair_count(Sim* s, int64_t* ordered_pairs_host, int64_t* nonzero_pairs_host);
 int k2_reference_forces(Sim* s, bool with_energy);     // variant 1: thread per target (k2_force.cu)
 int k2_chunk_forces(Sim* s, bool with_energy, bool stats);  // variant 2: chunk kernel (k2_chunk.cu)
 // K3  k3_integrate.cu
