@@ -93,7 +93,7 @@ class ClockSampler:
         return out
 
 
-def cpu_baseline(cfg, budget_s, seed=1):
+def cpu_baseline(cfg, budget_s, seed=1, state=None):
     """The oracle as it stands, timed on the host cores on a bounded sample: forces + energies of n_sample
     targets against ALL N sources (the all-pairs definition), scaled by N / n_sample to one force
     evaluation = one MD step (the O(N) integrator update is not in the sample; the force
@@ -103,7 +103,7 @@ def cpu_baseline(cfg, budget_s, seed=1):
     import oracle
 
     c = inputs.CONFIGS[cfg]
-    x, v, is_p, L = inputs.config_state(cfg, seed)
+    x, v, is_p, L = state if state is not None else inputs.config_state(cfg, seed)
     p = oracle.Params(r_c=c["r_c"])
     cores = oracle.num_threads()
     rng = np.random.default_rng(0)
@@ -135,8 +135,9 @@ def run_reference(args, rank, world):
     per_step = min(8.0, 150.0 / total)
     vals = []
     base = None
+    state = inputs.config_state(args.config, 1)
     for k in range(total):
-        base = cpu_baseline(args.config, per_step, seed=1)
+        base = cpu_baseline(args.config, per_step, seed=1, state=state)
         if k >= args.warmup:
             vals.append(base["value"])
     v = len(vals) / sum(1.0 / a for a in vals)
@@ -160,6 +161,21 @@ def workload_config(cfg, world):
         "N": c["N"], "parallelism": "replicas x%d (one GPU each, no data-path collective)" % world,
         "l2": "flushed between timed steps (256 MB write); the 50 MB MD state is otherwise L2-resident by nature",
     }
+
+
+def max_over_ranks(dev_s, e2e_s, dist, device="cuda"):
+    """The contract's timing rule: every number is the MAX over ranks (replicas run independently)."""
+    import torch
+
+    t = torch.tensor([dev_s, e2e_s], dtype=torch.float64, device=device)
+    if dist is not None:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return tuple(t.tolist())
+
+
+def aggregate_rate(world, steps, seconds):
+    """Whole-job steps/s of `world` independent replicas that each did `steps` steps in at most `seconds`."""
+    return world * steps / seconds
 
 
 def run_ours(args, rank, world, local_rank):
@@ -238,10 +254,7 @@ def run_ours(args, rank, world, local_rank):
     barrier()
     e2e_s = time.perf_counter() - t0
 
-    t = torch.tensor([dev_s, e2e_s], dtype=torch.float64, device="cuda")
-    if dist is not None:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    dev_s, e2e_s = t.tolist()
+    dev_s, e2e_s = max_over_ranks(dev_s, e2e_s, dist)
     if rank == 0:
         sm_max_mhz, hbm_gbs, peak_src = peaks()
         c_fp32, c_mufu = algorithmic_cost(c["Y_P"])
@@ -253,7 +266,7 @@ def run_ours(args, rank, world, local_rank):
         # (all pp pairs, np/nn pairs inside the underflow distance)
         achieved_nz = (17.0 * pairs_nz + 8.0 * c["Y_P"] ** 2 * pairs) / k2_s
         roof_pairs = min(fp32_peak / c_fp32, mufu_peak / c_mufu)
-        steps_per_s = world * args.steps / dev_s
+        steps_per_s = aggregate_rate(world, args.steps, dev_s)
         line = {
             "metric": "md_steps_per_s", "value": steps_per_s, "unit": "steps/s", "n_gpus": world,
             "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": 1e3 * dev_s / args.steps,
@@ -274,7 +287,7 @@ def run_ours(args, rank, world, local_rank):
                     SM_COUNT, FP32_LANES_PER_SM, sm_max_mhz, peak_src),
                 "traffic": None,
             },
-            "e2e": {"value": world * e2e_steps / e2e_s, "unit": "steps/s", "h2d_bytes_per_step": 72 * N,
+            "e2e": {"value": aggregate_rate(world, e2e_steps, e2e_s), "unit": "steps/s", "h2d_bytes_per_step": 72 * N,
                     "d2h_bytes_per_step": 72 * N, "steps": e2e_steps,
                     "what": "pasta_set_state_host(x,v,F) + pasta_step(1) + pasta_get_state_host(x,v,F), pinned host buffers"},
             "gpu_launches": launches, "wall_s": t_wall, "clocks": clocks,
@@ -291,8 +304,8 @@ def run_ours(args, rank, world, local_rank):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=100)
-    ap.add_argument("--warmup", type=int, default=10)
+    ap.add_argument("--steps", type=int, default=500)
+    ap.add_argument("--warmup", type=int, default=20)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", type=int, default=4, choices=[2, 4])
     ap.add_argument("--variant", type=int, default=None, help="pasta_params.force_variant override")

@@ -1,0 +1,37 @@
+"""bench.py's N > 1 leg is "replicas only": N independent simulations, one per rank, no
+data-path collective; the only cross-rank step is the max-over-ranks of the timed seconds.  That aggregation
+is covered here with world_size 2 on the gloo backend (CPU)."""
+import os
+import subprocess
+import sys
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+WORKER = r"""
+import os, sys, json
+sys.path.insert(0, %r)
+import torch, torch.distributed as dist
+import bench
+dist.init_process_group("gloo")
+rank = dist.get_rank()
+# rank r pretends its K steps took (1 + r) seconds on the device and 2 (1 + r) seconds end to end
+dev_s, e2e_s = bench.max_over_ranks(1.0 + rank, 2.0 * (1.0 + rank), dist, device="cpu")
+if rank == 0:
+    print(json.dumps({"dev_s": dev_s, "e2e_s": e2e_s, "value": bench.aggregate_rate(dist.get_world_size(), 10, dev_s)}))
+dist.destroy_process_group()
+"""
+
+
+def test_replica_aggregation_world_size_2(tmp_path):
+    script = tmp_path / "worker.py"
+    script.write_text(WORKER % ROOT)
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node=2", "--master-addr", "127.0.0.1",
+           "--master-port", "29533", str(script)]
+    out = subprocess.run(cmd, capture_output=True, text=True, timeout=240, env=dict(os.environ, OMP_NUM_THREADS="1"))
+    assert out.returncode == 0, out.stderr[-2000:]
+    import json
+
+    line = [l for l in out.stdout.splitlines() if l.startswith("{")][-1]
+    d = json.loads(line)
+    assert d["dev_s"] == 2.0 and d["e2e_s"] == 4.0          # max over the two ranks
+    assert d["value"] == 2 * 10 / 2.0                        # whole-job steps/s: all replicas' steps / slowest rank

@@ -325,3 +325,35 @@ def test_full_size_sampled_targets(orc, cfg):
         assert np.array_equal(_np(cid), cid_o) and np.array_equal(_np(start), start_o)
         sim.step(2, c["dt"])
         assert sim.step_count() == 2
+
+
+@pytest.mark.parametrize("N,density,r_c,Y_P", [(2048, 0.05, 17.0, 0.3), (30000, 0.08, 20.0, 0.4)])
+def test_exact_zero_skipping_changes_nothing_that_matters(orc, N, density, r_c, Y_P):
+    """skip_exact_zeros (D23): np/nn candidates beyond the FP32 underflow distance of exp2(-r'^2) are not
+    streamed.  Their terms are exactly 0.0f, so both settings must meet the oracle, and differ from each other
+    only by the rounding of FP32 partial sums taken in a different order."""
+    x, v, is_p, L = inputs.uniform_state(N, Y_P, density, 1.0, seed=11)
+    res = []
+    for skip in (1, 0):
+        with _sim_from_arrays(x, v, is_p, L, r_c=r_c, skip_exact_zeros=skip) as sim:
+            F, pe = sim.forces()
+            res.append((_np(F), pe))
+            if skip:
+                pairs, nonzero = sim.pair_counts()
+    Fo, _, peo, d = orc.forces(x, is_p, L, orc.Params(r_c=r_c))
+    for F, pe in res:
+        _check_forces(F, Fo, pe, peo)
+    assert np.linalg.norm(res[0][0] - res[1][0]) <= 2e-6 * np.linalg.norm(Fo)
+    assert abs(res[0][1] - res[1][1]) <= 1e-7 * abs(peo)
+    # the counters: in-range pairs as the oracle counts them (a pair within 1e-5 of r_c may flip, D22); the
+    # nonzero ones = pp pairs + np/nn pairs with r^2 log2(e) / (2 Lambda) < 126, counted here by brute force
+    assert abs(pairs - d["ordered_pairs"]) <= 4
+    if N <= 4096:
+        dx = x[:, None, :] - x[None, :, :]
+        dx -= L * np.round(dx / L)
+        r2 = (dx ** 2).sum(-1)
+        inr = (r2 < r_c ** 2) & ~np.eye(N, dtype=bool)
+        pp = np.outer(is_p, is_p).astype(bool)
+        nz = inr & (pp | (r2 * (math.log2(math.e) / 2.5) < 126.0))
+        assert abs(nonzero - int(nz.sum())) <= 4
+    assert nonzero <= pairs
