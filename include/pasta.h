@@ -58,7 +58,7 @@ typedef struct pasta_params {
   int32_t energy_every_step;   /* 1 (default): pasta_step evaluates per-particle energies with the forces */
   int32_t auto_grid;           /* 1 (default): each species' force grid picks its own k (about 8 particles per cell);
                                   0: both use cell_subdiv.  pasta_cells always reports the cell_subdiv grid */
-  int32_t x_subdiv;            /* thin cells along x per force-grid cell (0 = library default, 8) */
+  int32_t x_subdiv;            /* thin cells along x per force-grid cell (0 = library default: 8, fewer for a sparse species) */
   int32_t skip_exact_zeros;    /* 1 (default): np/nn candidates beyond the distance at which exp2(-r^2 log2e/2 Lambda)
                                   underflows FP32 (14.78 fm for Lambda = 1.25) are not streamed: their terms are exactly
                                   0.0f in the kernel's arithmetic, so F and e are unchanged (D23).  0: stream to r_c */

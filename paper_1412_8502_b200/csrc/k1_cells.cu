@@ -207,12 +207,86 @@ __global__ void k1_gather_kernel(int64_t N, const double* __restrict__ x, const 
   cxyz[t] = cx | (cy << 12) | (cz << 22);
 }
 
+// Chunk table of the pair kernel.  A chunk = the targets of one warp = consecutive sorted slots of ONE row of one
+// species, at most CHUNK_T of them, spanning fewer than xmax thin cells.  (A chunk that straddled two rows, or 8
+// far-apart particles of a sparse or clustered species, would have a huge bounding box and large frame
+// coordinates.)  NOMINAL chunks are the stretches [row start + 8 k, row start + 8 k + 8) of every row; a nominal
+// chunk is cut further, greedily, wherever the extent limit is reached (in a dense system: never).  One thread
+// handles the nominal chunks that START in the slots [8 j, 8 j + 8): it needs the cell coordinates of 16 slots
+// and the first slot of the row of slot 8 j.  Entry = first slot | targets << 26.
+constexpr int CHUNK_T = 8;
+struct ChunkGeom {
+  int xmax[2];
+};
+
+__global__ void k1_chunk_table_kernel(int32_t N, int32_t Np, const int32_t* __restrict__ cxyz,
+                                      const int32_t* __restrict__ bin_start, const GridPair g, const ChunkGeom cg,
+                                      int32_t* __restrict__ chunk_tab, int32_t* __restrict__ n_overflow) {
+  const int j = blockIdx.x * blockDim.x + threadIdx.x;
+  const int lo = j * CHUNK_T;
+  // row key of a slot: species and (cy, cz); -1 beyond the end
+  int c[2 * CHUNK_T], key[2 * CHUNK_T];
+#pragma unroll
+  for (int k = 0; k < 2 * CHUNK_T; ++k) {
+    const int p = lo + k;
+    c[k] = p < N ? __ldg(cxyz + p) : 0;
+    key[k] = p < N ? ((c[k] >> 12) | (p < Np ? 0 : (1 << 24))) : -1;
+  }
+  // first slot of the row that slot `lo` belongs to
+  const int sp0 = lo < Np ? 0 : 1;
+  int row_lo = lo >= N ? 0 : __ldg(bin_start + g.base[sp0] + (PASTA_CZ(c[0]) * g.ncell[sp0] + PASTA_CY(c[0])) * g.ncx[sp0]);
+  int entry[CHUNK_T];
+  int m = 0;
+#pragma unroll
+  for (int k = 0; k < CHUNK_T; ++k) {
+    if (key[k] < 0) break;
+    if (k > 0 && key[k] != key[k - 1]) row_lo = lo + k;  // sorted: the first slot with a new key starts its row
+    if (((lo + k - row_lo) & (CHUNK_T - 1)) != 0) continue;
+    // nominal chunk [lo + k, lo + k + 8) within the row; cut it where the extent limit is reached
+    const int xm = cg.xmax[(key[k] >> 24) & 1];
+    int first = k;
+#pragma unroll
+    for (int q = 1; q <= CHUNK_T; ++q) {
+      const bool end = q == CHUNK_T || key[k + q] != key[k];
+      if (end || PASTA_CX(c[k + q]) - PASTA_CX(c[first]) >= xm) {
+        entry[m++] = (lo + first) | ((k + q - first) << 26);
+        first = k + q;
+      }
+      if (end) break;
+    }
+  }
+  // entry j of the table = the first chunk found (in slot order: neighbouring warps of the pair kernel work on
+  // neighbouring chunks of a row and share their sources in L1; 0 = none); further ones go to the overflow
+  // region behind the ceil(N / 8) primary entries
+  if (lo < N) {
+    chunk_tab[j] = m > 0 ? entry[0] : 0;
+    if (m > 1) {
+      const int at = (N + CHUNK_T - 1) / CHUNK_T + atomicAdd(n_overflow, m - 1);
+      for (int k = 1; k < m; ++k) chunk_tab[at + k - 1] = entry[k];
+    }
+  }
+}
+
 // Cells per side of a species' grid: the O3 formula with the k that puts about CHUNK particles in a cell.
 static int auto_subdiv(double L, double r_c, int64_t n_species, int k_default) {
   if (n_species <= 0) return k_default;
   const double w_star = L * cbrt(8.0 / (double)n_species);
   int k = (int)floor(r_c / w_star + 0.5);
+  // never wider than 8 fm: sorted coordinates are FP32 offsets from the cell centre, and their quantum
+  // (2^-24 of the half width) times the steepest pair-force gradient (~80 MeV/fm^2 inside a cluster) has to
+  // stay below the force tolerance
+  const int k_min = (int)ceil(r_c / 8.0);
+  k = k < k_min ? k_min : k;
   return k < 1 ? 1 : (k > 64 ? 64 : k);
+}
+
+// Thin cells along x per cell: 8 where the species is dense; fewer where the grid would otherwise have many more
+// bins than the species has particles (a sparse species: the bin tables, not the particles, would set the cost).
+static int auto_xsub(double L, double r_c, int k, int64_t n_species) {
+  const double ncell = floor(L * (double)k / r_c);
+  int xsub = 8;
+  while (xsub > 1 && ncell * ncell * ncell * xsub > 4.0 * (double)n_species + 65536.0) xsub /= 2;
+  return xsub;
 }
 
 int k1_build(Sim* s, bool uniform_grid) {
@@ -223,9 +297,10 @@ int k1_build(Sim* s, bool uniform_grid) {
   const bool same_k = uniform || s->prm.auto_grid == 0;
   const int k0 = same_k ? s->prm.cell_subdiv : auto_subdiv(s->L, s->prm.r_c, s->Np, s->prm.cell_subdiv);
   const int k1 = same_k ? s->prm.cell_subdiv : auto_subdiv(s->L, s->prm.r_c, N - s->Np, s->prm.cell_subdiv);
-  const int xsub = uniform ? 1 : (s->prm.x_subdiv > 0 ? s->prm.x_subdiv : 8);
-  s->grid_sp[0] = make_grid(s->L, s->prm.r_c, k0, xsub);
-  s->grid_sp[1] = make_grid(s->L, s->prm.r_c, k1, xsub);
+  const int xs0 = uniform ? 1 : (s->prm.x_subdiv > 0 ? s->prm.x_subdiv : auto_xsub(s->L, s->prm.r_c, k0, s->Np));
+  const int xs1 = uniform ? 1 : (s->prm.x_subdiv > 0 ? s->prm.x_subdiv : auto_xsub(s->L, s->prm.r_c, k1, N - s->Np));
+  s->grid_sp[0] = make_grid(s->L, s->prm.r_c, k0, xs0);
+  s->grid_sp[1] = make_grid(s->L, s->prm.r_c, k1, xs1);
   GridPair g;
   for (int sp = 0; sp < 2; ++sp) {
     g.ncell[sp] = s->grid_sp[sp].ncell;
@@ -257,6 +332,30 @@ int k1_build(Sim* s, bool uniform_grid) {
                                                         s->perm.as<int32_t>(), g, sigma, s->pos4.as<float4>(),
                                                         s->cxyz.as<int32_t>());
   s->launches += 3;
+  if (!uniform) {
+    // extent limit of a chunk: three cell widths, at most 16 fm; and an upper bound of the number of chunks
+    // (cuts at multiples of 8 slots: N / 8; at row or species changes: one per row; at the extent limit:
+    // at most ncx / xmax + 1 per row, because such chunks cover disjoint stretches of >= xmax thin cells)
+    ChunkGeom cg;
+    int64_t bound = (N + CHUNK_T - 1) / CHUNK_T + 1;
+    int64_t rows = 0;
+    for (int sp = 0; sp < 2; ++sp) {
+      const Grid& gr = s->grid_sp[sp];
+      int xm = (int)floor(fmin(3.0 * gr.w, 16.0) / gr.wx);
+      cg.xmax[sp] = xm < 1 ? 1 : xm;
+      const int64_t nrow = (int64_t)gr.ncell * gr.ncell;
+      rows += nrow;
+      bound += nrow * (gr.ncx / cg.xmax[sp] + 2);
+    }
+    if (bound > N + rows) bound = N + rows;
+    s->max_chunks = bound;
+    PASTA_TRY(buffer_reserve(s, &s->chunk_tab, sizeof(int32_t) * (size_t)(bound + 64)));
+    int32_t* n_chunks = s->counters.as<int32_t>() + 2 * 24;
+    PASTA_CUDA_OK(cudaMemsetAsync(n_chunks, 0, sizeof(int32_t), s->stream));
+    k1_chunk_table_kernel<<<grid_for((N + CHUNK_T - 1) / CHUNK_T, 128), 128, 0, s->stream>>>(
+        (int32_t)N, (int32_t)s->Np, s->cxyz.as<int32_t>(), start, g, cg, s->chunk_tab.as<int32_t>(), n_chunks);
+    s->launches += 1;
+  }
   PASTA_CUDA_OK(cudaGetLastError());
   return PASTA_OK;
 }

@@ -72,7 +72,9 @@ struct SpeciesGrid {
 
 struct ChunkArgs {
   int32_t N, Np;
-  int32_t n_chunks_p, n_chunks;
+  const int32_t* chunk_tab;  // [chunk] first slot | number of targets << 26 (k1_chunk_table_kernel)
+  const int32_t* counts;     // [0] number of chunks in the overflow region
+  int32_t nprim;             // primary entries: ceil(N / 8), some of them empty
   SpeciesGrid g[2];
   float rcS;     // sigma * r_c
   float rzeroS;  // scaled distance beyond which exp2(-r'^2) is exactly 0 in FP32 with FTZ (sqrt(126.5))
@@ -332,39 +334,23 @@ __device__ __forceinline__ int min_image_cells(int m, int nc) {
   return m + (m > hc ? -nc : (m < -hc ? nc : 0));
 }
 
+// Both passes of one chunk.  The chunk table (k1_chunk_table_kernel) makes every chunk COMPACT: its targets lie in
+// one row, fewer than xmax thin cells apart.  In a dense system that is 8 consecutive particles of a row (they
+// span about one cell width); where a species is sparse or clustered the table cuts chunks short instead, which
+// keeps the bounding box tight (few wasted candidates) and the frame coordinates small (FP32 ulp of a
+// displacement <= 1e-6 fm).  The frame's origin cell is the middle of the chunk's extent.
 template <bool CUT, bool ENERGY, bool STATS>
-__global__ void __launch_bounds__(WARPS * 32, K2_MINB) k2_chunk_kernel(const ChunkArgs A, const PairConsts c) {
-  __shared__ WarpShared shared[WARPS];
-  const int lane = threadIdx.x & 31;
-  // the warp index is produced by REDUX so that the compiler can prove it warp-uniform and keep it (and
-  // everything derived from it) in uniform registers, off the vector register file
-  const int wib = __reduce_or_sync(0xffffffffu, (int)(threadIdx.x >> 5));
-  const int pr = lane / NPH, ph = lane % NPH;  // this lane's target pair and phase
-  const int chunk = blockIdx.x * WARPS + wib;
-  if (chunk >= A.n_chunks) return;
-  WarpShared& sh = shared[wib];
-
-  const bool chunk_p = chunk < A.n_chunks_p;
-  const int st_sp = chunk_p ? 0 : 1;
-  const SpeciesGrid gt = A.g[st_sp];
-  const int base = chunk_p ? chunk * T : A.Np + (chunk - A.n_chunks_p) * T;
-  const int nvalid = min(T, (chunk_p ? A.Np : A.N) - base);
-
-  // ---- targets: lane l < nvalid holds target l; all other lanes mirror target 0 ------------------------
-  const int tl = lane < nvalid ? lane : 0;
-  const float4 tp = __ldg(A.pos4 + base + tl);
-  const int tc = __ldg(A.cxyz + base + tl);
-  const int oc = __shfl_sync(0xffffffffu, tc, 0);
-  const int ox = PASTA_CX(oc), oy = PASTA_CY(oc), oz = PASTA_CZ(oc);
-  // cell offset from the origin cell, taken in the nearest periodic image (chunks may wrap a row end)
-  const int mx = min_image_cells(PASTA_CX(tc) - ox, gt.ncx);
-  const int my = min_image_cells(PASTA_CY(tc) - oy, gt.ncell);
-  const int mz = min_image_cells(PASTA_CZ(tc) - oz, gt.ncell);
-
-  Accum acc;
-  acc.fx = acc.fy = acc.fz = acc.e = acc.s1 = acc.s2 = make_float2(0.f, 0.f);
-  unsigned long long st[3] = {0, 0, 0};
-
+__device__ __forceinline__ void chunk_passes(const ChunkArgs& A, const PairConsts& c, WarpShared& sh, const int lane,
+                                             const int pr, const SpeciesGrid& gt, const int st_sp, const bool chunk_p,
+                                             const float4 tp, const int tc, const int nvalid, Accum& acc,
+                                             unsigned long long* st) {
+  const int c_first = __shfl_sync(0xffffffffu, tc, 0), c_last = __shfl_sync(0xffffffffu, tc, nvalid - 1);
+  const int oy = PASTA_CY(c_first), oz = PASTA_CZ(c_first);
+  const int ox = PASTA_CX(c_first) + (PASTA_CX(c_last) - PASTA_CX(c_first)) / 2;  // sorted by cx within the row
+  const int mx = PASTA_CX(tc) - ox, my = 0, mz = 0;
+  const bool mine = lane < nvalid;
+  const unsigned active = nvalid >= 32 ? 0xffffffffu : ((1u << nvalid) - 1u);
+  const int j0 = 0;
   // ---- pass 0: proton sources, pass 1: neutron sources -------------------------------------------------
 #pragma unroll
   for (int sp = 0; sp < 2; ++sp) {
@@ -387,7 +373,14 @@ __global__ void __launch_bounds__(WARPS * 32, K2_MINB) k2_chunk_kernel(const Chu
       Y = (float)((double)tp.y + (double)my * gt.wS_d + (cy0 - ((double)ry + 0.5) * gs.wS_d));
       Z = (float)((double)tp.z + (double)mz * gt.wS_d + (cz0 - ((double)rz + 0.5) * gs.wS_d));
     }
-    // bounding box of the chunk (lanes >= nvalid mirror target 0)
+    // bounding box of the round's targets (every other lane mirrors the first one)
+    {
+      const float Xo = __shfl_sync(0xffffffffu, X, j0), Yo = __shfl_sync(0xffffffffu, Y, j0),
+                  Zo = __shfl_sync(0xffffffffu, Z, j0);
+      X = mine ? X : Xo;
+      Y = mine ? Y : Yo;
+      Z = mine ? Z : Zo;
+    }
     Box b = {X, X, Y, Y, Z, Z};
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) {
@@ -404,7 +397,7 @@ __global__ void __launch_bounds__(WARPS * 32, K2_MINB) k2_chunk_kernel(const Chu
       const float x0 = __shfl_sync(0xffffffffu, X, 2 * pr), x1 = __shfl_sync(0xffffffffu, X, 2 * pr + 1);
       const float y0 = __shfl_sync(0xffffffffu, Y, 2 * pr), y1 = __shfl_sync(0xffffffffu, Y, 2 * pr + 1);
       const float z0 = __shfl_sync(0xffffffffu, Z, 2 * pr), z1 = __shfl_sync(0xffffffffu, Z, 2 * pr + 1);
-      const bool v0 = 2 * pr < nvalid, v1 = 2 * pr + 1 < nvalid;
+      const bool v0 = ((active >> (2 * pr)) & 1u) != 0, v1 = ((active >> (2 * pr + 1)) & 1u) != 0;
       t.ntx = make_float2(v0 ? -x0 : FAR, v1 ? -x1 : FAR);
       t.nty = make_float2(v0 ? -y0 : FAR, v1 ? -y1 : FAR);
       t.ntz = make_float2(v0 ? -z0 : FAR, v1 ? -z1 : FAR);
@@ -424,6 +417,37 @@ __global__ void __launch_bounds__(WARPS * 32, K2_MINB) k2_chunk_kernel(const Chu
       acc.s1 = acc.s2 = make_float2(0.f, 0.f);
     }
   }
+}
+
+template <bool CUT, bool ENERGY, bool STATS>
+__global__ void __launch_bounds__(WARPS * 32, K2_MINB) k2_chunk_kernel(const ChunkArgs A, const PairConsts c) {
+  __shared__ WarpShared shared[WARPS];
+  const int lane = threadIdx.x & 31;
+  // the warp index is produced by REDUX so that the compiler can prove it warp-uniform and keep it (and
+  // everything derived from it) in uniform registers, off the vector register file
+  const int wib = __reduce_or_sync(0xffffffffu, (int)(threadIdx.x >> 5));
+  const int pr = lane / NPH, ph = lane % NPH;  // this lane's target pair and phase
+  const int chunk = blockIdx.x * WARPS + wib;
+  if (chunk >= A.nprim + A.counts[0]) return;  // the launch covers an upper bound of the number of chunks
+  WarpShared& sh = shared[wib];
+
+  const int entry = __ldg(A.chunk_tab + chunk);
+  const int base = entry & 0x3ffffff, nvalid = entry >> 26;
+  if (nvalid == 0) return;  // empty primary entry
+  const bool chunk_p = base < A.Np;
+  const int st_sp = chunk_p ? 0 : 1;
+  const SpeciesGrid& gt = A.g[st_sp];
+
+  // ---- targets: lane l < nvalid holds target l ------------------------------------------------------------
+  const int tl = lane < nvalid ? lane : 0;
+  const float4 tp = __ldg(A.pos4 + base + tl);
+  const int tc = __ldg(A.cxyz + base + tl);
+
+  Accum acc;
+  acc.fx = acc.fy = acc.fz = acc.e = acc.s1 = acc.s2 = make_float2(0.f, 0.f);
+  unsigned long long st[3] = {0, 0, 0};
+
+  chunk_passes<CUT, ENERGY, STATS>(A, c, sh, lane, pr, gt, st_sp, chunk_p, tp, tc, nvalid, acc, st);
 
   // ---- combine the phases' FP32 partials in FP64 ------------------------------------------------------------
   // quantity index q = 4 * (target within the pair) + {fx, fy, fz, e}; a transposing butterfly over the
@@ -487,8 +511,9 @@ int k2_chunk_forces(Sim* s, bool with_energy, bool stats) {
   ChunkArgs A;
   A.N = (int32_t)s->N;
   A.Np = (int32_t)s->Np;
-  A.n_chunks_p = (int32_t)((s->Np + T - 1) / T);
-  A.n_chunks = A.n_chunks_p + (int32_t)((s->N - s->Np + T - 1) / T);
+  A.chunk_tab = s->chunk_tab.as<int32_t>();
+  A.counts = s->counters.as<int32_t>() + 2 * 24;
+  A.nprim = (int32_t)((s->N + T - 1) / T);
   for (int sp = 0; sp < 2; ++sp) {
     const Grid& g = s->grid_sp[sp];
     A.g[sp].ncell = g.ncell;
@@ -512,19 +537,21 @@ int k2_chunk_forces(Sim* s, bool with_energy, bool stats) {
   A.stats = s->counters.as<unsigned long long>() + 10;
   // exp2(-r'^2) is exactly 0 (FTZ) for r'^2 > 126: then np/nn pairs beyond r_c need no explicit cut
   const bool cut = (double)c.rc2s < 127.0;
-  const int grid = (A.n_chunks + WARPS - 1) / WARPS;
+  const int grid = (int)((s->max_chunks + WARPS - 1) / WARPS);
   const dim3 block(WARPS * 32);
+  if (stats) PASTA_CUDA_OK(cudaMemsetAsync(A.stats, 0, 3 * sizeof(unsigned long long), s->stream));
+#define PASTA_K2_LAUNCH(CUT_, EN_, ST_) k2_chunk_kernel<CUT_, EN_, ST_><<<grid, block, 0, s->stream>>>(A, c)
   if (stats) {
-    PASTA_CUDA_OK(cudaMemsetAsync(A.stats, 0, 3 * sizeof(unsigned long long), s->stream));
-    if (cut) k2_chunk_kernel<true, true, true><<<grid, block, 0, s->stream>>>(A, c);
-    else k2_chunk_kernel<false, true, true><<<grid, block, 0, s->stream>>>(A, c);
+    if (cut) PASTA_K2_LAUNCH(true, true, true);
+    else PASTA_K2_LAUNCH(false, true, true);
   } else if (with_energy) {
-    if (cut) k2_chunk_kernel<true, true, false><<<grid, block, 0, s->stream>>>(A, c);
-    else k2_chunk_kernel<false, true, false><<<grid, block, 0, s->stream>>>(A, c);
+    if (cut) PASTA_K2_LAUNCH(true, true, false);
+    else PASTA_K2_LAUNCH(false, true, false);
   } else {
-    if (cut) k2_chunk_kernel<true, false, false><<<grid, block, 0, s->stream>>>(A, c);
-    else k2_chunk_kernel<false, false, false><<<grid, block, 0, s->stream>>>(A, c);
+    if (cut) PASTA_K2_LAUNCH(true, false, false);
+    else PASTA_K2_LAUNCH(false, false, false);
   }
+#undef PASTA_K2_LAUNCH
   s->launches += 1;
   PASTA_CUDA_OK(cudaGetLastError());
   return PASTA_OK;

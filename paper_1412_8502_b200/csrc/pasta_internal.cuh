@@ -109,8 +109,11 @@ struct Sim {
   Buffer cl_parent, cl_A, cl_Z;  // int32[N] each
   Buffer cl_cell_id, cl_count, cl_start, cl_perm;
 
-  // pair-force chunk tables (k2_force.cu)
-  Buffer chunk_aux;
+  // pair-force chunk table (k1_cells.cu -> k2_chunk.cu): [0, max_chunks) entries first slot | count << 26,
+  // [max_chunks, 2 max_chunks) the list of chunks that need several rounds; the counters live in
+  // counters[24] (int32 view [48]: number of chunks, [49]: length of that list)
+  Buffer chunk_tab;
+  int64_t max_chunks = 0;
 
   // timing: pairs of events (start, stop) tagged with the kernel group they bracket
   bool timing = false;
