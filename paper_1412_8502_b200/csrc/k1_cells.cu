@@ -207,23 +207,41 @@ __global__ void k1_gather_kernel(int64_t N, const double* __restrict__ x, const 
   cxyz[t] = cx | (cy << 12) | (cz << 22);
 }
 
-// Chunk table of the pair kernel.  A chunk = the targets of one warp = consecutive sorted slots of ONE row of one
-// species, at most CHUNK_T of them, spanning fewer than xmax thin cells.  (A chunk that straddled two rows, or 8
-// far-apart particles of a sparse or clustered species, would have a huge bounding box and large frame
-// coordinates.)  NOMINAL chunks are the stretches [row start + 8 k, row start + 8 k + 8) of every row; a nominal
-// chunk is cut further, greedily, wherever the extent limit is reached (in a dense system: never).  One thread
-// handles the nominal chunks that START in the slots [8 j, 8 j + 8): it needs the cell coordinates of 16 slots
-// and the first slot of the row of slot 8 j.  Entry = first slot | targets << 26.
+// Chunk table of the pair kernel.  A chunk = the targets of one warp = up to CHUNK_T sorted slots of one species
+// that are close together; an entry of the table lists its slots (-1 = none).  Two builders, chosen per species
+// by the mean number of particles per cell:
+//   DENSE  (row runs): NOMINAL chunks are the stretches [row start + 8 k, row start + 8 k + 8) of every row
+//          (a chunk never straddles two rows: the two parts would be a cell width apart in y or z and on
+//          opposite faces in x); a nominal chunk is cut further, greedily, wherever its extent reaches xmax thin
+//          cells (in a dense system: never).  One thread handles the nominal chunks that START in the slots
+//          [8 j, 8 j + 8): it needs the cell coordinates of 16 slots and the first slot of the row of slot 8 j.
+//          Entry j of the table is the first chunk it finds (so neighbouring warps of the pair kernel work on
+//          neighbouring chunks of a row and share their sources in L1; it may be empty), further ones go to the
+//          overflow region.
+//   SPARSE (blocks): 8 consecutive particles of a row would be far apart, so the particles of a block of B x B x B
+//          cells (B w <= 20 fm) are grouped instead, 8 at a time; one thread per block, entries in the overflow
+//          region, reserved once per warp.
 constexpr int CHUNK_T = 8;
 struct ChunkGeom {
-  int xmax[2];
+  int xmax[2];   // DENSE: extent limit of a chunk in thin cells
+  int block[2];  // 0 = DENSE, else B of the SPARSE builder
+  int nprim;     // primary entries
 };
 
-__global__ void k1_chunk_table_kernel(int32_t N, int32_t Np, const int32_t* __restrict__ cxyz,
-                                      const int32_t* __restrict__ bin_start, const GridPair g, const ChunkGeom cg,
-                                      int32_t* __restrict__ chunk_tab, int32_t* __restrict__ n_overflow) {
+__device__ __forceinline__ void write_entry(int32_t* __restrict__ tab, int64_t e, int first, int n) {
+  int4 a, b;
+  a.x = n > 0 ? first : -1; a.y = n > 1 ? first + 1 : -1; a.z = n > 2 ? first + 2 : -1; a.w = n > 3 ? first + 3 : -1;
+  b.x = n > 4 ? first + 4 : -1; b.y = n > 5 ? first + 5 : -1; b.z = n > 6 ? first + 6 : -1; b.w = n > 7 ? first + 7 : -1;
+  reinterpret_cast<int4*>(tab + e * CHUNK_T)[0] = a;
+  reinterpret_cast<int4*>(tab + e * CHUNK_T)[1] = b;
+}
+
+__global__ void k1_chunk_rows_kernel(int32_t N, int32_t Np, const int32_t* __restrict__ cxyz,
+                                     const int32_t* __restrict__ bin_start, const GridPair g, const ChunkGeom cg,
+                                     int32_t* __restrict__ chunk_tab, int32_t* __restrict__ n_overflow) {
   const int j = blockIdx.x * blockDim.x + threadIdx.x;
   const int lo = j * CHUNK_T;
+  if (lo >= N) return;
   // row key of a slot: species and (cy, cz); -1 beyond the end
   int c[2 * CHUNK_T], key[2 * CHUNK_T];
 #pragma unroll
@@ -234,37 +252,76 @@ __global__ void k1_chunk_table_kernel(int32_t N, int32_t Np, const int32_t* __re
   }
   // first slot of the row that slot `lo` belongs to
   const int sp0 = lo < Np ? 0 : 1;
-  int row_lo = lo >= N ? 0 : __ldg(bin_start + g.base[sp0] + (PASTA_CZ(c[0]) * g.ncell[sp0] + PASTA_CY(c[0])) * g.ncx[sp0]);
-  int entry[CHUNK_T];
+  int row_lo = __ldg(bin_start + g.base[sp0] + (PASTA_CZ(c[0]) * g.ncell[sp0] + PASTA_CY(c[0])) * g.ncx[sp0]);
+  int first_slot[CHUNK_T], count[CHUNK_T];
   int m = 0;
 #pragma unroll
   for (int k = 0; k < CHUNK_T; ++k) {
     if (key[k] < 0) break;
     if (k > 0 && key[k] != key[k - 1]) row_lo = lo + k;  // sorted: the first slot with a new key starts its row
     if (((lo + k - row_lo) & (CHUNK_T - 1)) != 0) continue;
+    const int sp = (key[k] >> 24) & 1;
+    if (cg.block[sp] != 0) continue;  // this species is grouped by blocks
     // nominal chunk [lo + k, lo + k + 8) within the row; cut it where the extent limit is reached
-    const int xm = cg.xmax[(key[k] >> 24) & 1];
+    const int xm = cg.xmax[sp];
     int first = k;
 #pragma unroll
     for (int q = 1; q <= CHUNK_T; ++q) {
       const bool end = q == CHUNK_T || key[k + q] != key[k];
       if (end || PASTA_CX(c[k + q]) - PASTA_CX(c[first]) >= xm) {
-        entry[m++] = (lo + first) | ((k + q - first) << 26);
+        first_slot[m] = lo + first;
+        count[m++] = k + q - first;
         first = k + q;
       }
       if (end) break;
     }
   }
-  // entry j of the table = the first chunk found (in slot order: neighbouring warps of the pair kernel work on
-  // neighbouring chunks of a row and share their sources in L1; 0 = none); further ones go to the overflow
-  // region behind the ceil(N / 8) primary entries
-  if (lo < N) {
-    chunk_tab[j] = m > 0 ? entry[0] : 0;
-    if (m > 1) {
-      const int at = (N + CHUNK_T - 1) / CHUNK_T + atomicAdd(n_overflow, m - 1);
-      for (int k = 1; k < m; ++k) chunk_tab[at + k - 1] = entry[k];
-    }
+  write_entry(chunk_tab, j, m > 0 ? first_slot[0] : 0, m > 0 ? count[0] : 0);
+  if (m > 1) {
+    const int at = cg.nprim + atomicAdd(n_overflow, m - 1);
+    for (int k = 1; k < m; ++k) write_entry(chunk_tab, at + k - 1, first_slot[k], count[k]);
   }
+}
+
+__global__ void k1_chunk_blocks_kernel(int sp, const int32_t* __restrict__ bin_start, const GridPair g,
+                                       const ChunkGeom cg, int32_t* __restrict__ chunk_tab,
+                                       int32_t* __restrict__ n_overflow) {
+  const int B = cg.block[sp], nc = g.ncell[sp], ncx = g.ncx[sp], xs = ncx / nc;
+  const int nb = (nc + B - 1) / B;
+  const int t = blockIdx.x * blockDim.x + threadIdx.x;
+  const bool live = t < nb * nb * nb;
+  const int bx = t % nb, by = (t / nb) % nb, bz = t / (nb * nb);
+  const int x0 = bx * B * xs, x1 = min(x0 + B * xs, ncx);
+  int total = 0;
+  if (live)
+    for (int cz = bz * B; cz < min(bz * B + B, nc); ++cz)
+      for (int cy = by * B; cy < min(by * B + B, nc); ++cy) {
+        const int32_t* bs = bin_start + g.base[sp] + (cz * nc + cy) * ncx;
+        total += __ldg(bs + x1) - __ldg(bs + x0);
+      }
+  const int m = (total + CHUNK_T - 1) / CHUNK_T;
+  // one reservation per warp
+  const int lane = threadIdx.x & 31;
+  int incl = m;
+#pragma unroll
+  for (int o = 1; o < 32; o <<= 1) {
+    const int v = __shfl_up_sync(0xffffffffu, incl, o);
+    if (lane >= o) incl += v;
+  }
+  const int wtotal = __shfl_sync(0xffffffffu, incl, 31);
+  int at = 0;
+  if (lane == 0 && wtotal > 0) at = atomicAdd(n_overflow, wtotal);
+  at = cg.nprim + __shfl_sync(0xffffffffu, at, 0) + incl - m;
+  if (m == 0) return;
+  int32_t* out = chunk_tab + (int64_t)at * CHUNK_T;
+  int k = 0;
+  for (int cz = bz * B; cz < min(bz * B + B, nc); ++cz)
+    for (int cy = by * B; cy < min(by * B + B, nc); ++cy) {
+      const int32_t* bs = bin_start + g.base[sp] + (cz * nc + cy) * ncx;
+      const int hi = __ldg(bs + x1);
+      for (int p = __ldg(bs + x0); p < hi; ++p) out[k++] = p;
+    }
+  for (; k < m * CHUNK_T; ++k) out[k] = -1;
 }
 
 // Cells per side of a species' grid: the O3 formula with the k that puts about CHUNK particles in a cell.
@@ -333,28 +390,55 @@ int k1_build(Sim* s, bool uniform_grid) {
                                                         s->cxyz.as<int32_t>());
   s->launches += 3;
   if (!uniform) {
-    // extent limit of a chunk: three cell widths, at most 16 fm; and an upper bound of the number of chunks
-    // (cuts at multiples of 8 slots: N / 8; at row or species changes: one per row; at the extent limit:
-    // at most ncx / xmax + 1 per row, because such chunks cover disjoint stretches of >= xmax thin cells)
+    // builder per species (DENSE row runs: at least 3 particles per cell on average), the extent limit of a row
+    // run (three cell widths, at most 16 fm) and the capacity of the table: a bound on the number of chunks
+    //   row runs: primary entries ceil(N / 8); overflow <= one per row (row or species change inside 8 slots)
+    //             + ncx / xmax + 1 per row (runs cut at the extent limit cover disjoint stretches >= xmax)
+    //   blocks:   n / 8 + one per block
     ChunkGeom cg;
-    int64_t bound = (N + CHUNK_T - 1) / CHUNK_T + 1;
-    int64_t rows = 0;
+    int64_t overflow = 64;
+    bool any_rows = false;
     for (int sp = 0; sp < 2; ++sp) {
       const Grid& gr = s->grid_sp[sp];
+      const int64_t n_sp = sp == 0 ? s->Np : N - s->Np;
+      const double occ = (double)n_sp / ((double)gr.ncell * gr.ncell * gr.ncell);
       int xm = (int)floor(fmin(3.0 * gr.w, 16.0) / gr.wx);
       cg.xmax[sp] = xm < 1 ? 1 : xm;
+      cg.block[sp] = 0;
+      if (occ < 3.0 && gr.ncell >= 4) {
+        int B = (int)ceil(cbrt(8.0 / fmax(occ, 1e-9)));
+        const int Bmax = (int)floor(20.0 / gr.w);
+        B = B > 3 ? 3 : B;
+        B = B > Bmax ? Bmax : B;
+        cg.block[sp] = B < 1 ? 1 : B;
+      }
       const int64_t nrow = (int64_t)gr.ncell * gr.ncell;
-      rows += nrow;
-      bound += nrow * (gr.ncx / cg.xmax[sp] + 2);
+      if (cg.block[sp] == 0) {
+        any_rows = any_rows || n_sp > 0;
+        overflow += nrow * (gr.ncx / cg.xmax[sp] + 2);
+      } else {
+        const int64_t nb = (gr.ncell + cg.block[sp] - 1) / cg.block[sp];
+        overflow += n_sp / CHUNK_T + nb * nb * nb;
+      }
     }
-    if (bound > N + rows) bound = N + rows;
-    s->max_chunks = bound;
-    PASTA_TRY(buffer_reserve(s, &s->chunk_tab, sizeof(int32_t) * (size_t)(bound + 64)));
-    int32_t* n_chunks = s->counters.as<int32_t>() + 2 * 24;
-    PASTA_CUDA_OK(cudaMemsetAsync(n_chunks, 0, sizeof(int32_t), s->stream));
-    k1_chunk_table_kernel<<<grid_for((N + CHUNK_T - 1) / CHUNK_T, 128), 128, 0, s->stream>>>(
-        (int32_t)N, (int32_t)s->Np, s->cxyz.as<int32_t>(), start, g, cg, s->chunk_tab.as<int32_t>(), n_chunks);
-    s->launches += 1;
+    cg.nprim = any_rows ? (int)((N + CHUNK_T - 1) / CHUNK_T) : 0;
+    s->chunk_nprim = cg.nprim;
+    s->max_chunks = cg.nprim + overflow;
+    PASTA_TRY(buffer_reserve(s, &s->chunk_tab, sizeof(int32_t) * CHUNK_T * (size_t)(s->max_chunks + 8)));
+    int32_t* n_overflow = s->counters.as<int32_t>() + 2 * 24;
+    PASTA_CUDA_OK(cudaMemsetAsync(n_overflow, 0, sizeof(int32_t), s->stream));
+    if (any_rows) {
+      k1_chunk_rows_kernel<<<grid_for(cg.nprim, 128), 128, 0, s->stream>>>(
+          (int32_t)N, (int32_t)s->Np, s->cxyz.as<int32_t>(), start, g, cg, s->chunk_tab.as<int32_t>(), n_overflow);
+      s->launches += 1;
+    }
+    for (int sp = 0; sp < 2; ++sp)
+      if (cg.block[sp] != 0 && (sp == 0 ? s->Np : N - s->Np) > 0) {
+        const int64_t nb = (s->grid_sp[sp].ncell + cg.block[sp] - 1) / cg.block[sp];
+        k1_chunk_blocks_kernel<<<grid_for(nb * nb * nb, 128), 128, 0, s->stream>>>(sp, start, g, cg,
+                                                                                   s->chunk_tab.as<int32_t>(), n_overflow);
+        s->launches += 1;
+      }
   }
   PASTA_CUDA_OK(cudaGetLastError());
   return PASTA_OK;

@@ -72,9 +72,9 @@ struct SpeciesGrid {
 
 struct ChunkArgs {
   int32_t N, Np;
-  const int32_t* chunk_tab;  // [chunk] first slot | number of targets << 26 (k1_chunk_table_kernel)
+  const int32_t* chunk_tab;  // [chunk][8] sorted slots of the chunk's targets, -1 = none (k1_cells.cu)
   const int32_t* counts;     // [0] number of chunks in the overflow region
-  int32_t nprim;             // primary entries: ceil(N / 8), some of them empty
+  int32_t nprim;             // primary entries (some of them empty)
   SpeciesGrid g[2];
   float rcS;     // sigma * r_c
   float rzeroS;  // scaled distance beyond which exp2(-r'^2) is exactly 0 in FP32 with FTZ (sqrt(126.5))
@@ -334,23 +334,38 @@ __device__ __forceinline__ int min_image_cells(int m, int nc) {
   return m + (m > hc ? -nc : (m < -hc ? nc : 0));
 }
 
-// Both passes of one chunk.  The chunk table (k1_chunk_table_kernel) makes every chunk COMPACT: its targets lie in
-// one row, fewer than xmax thin cells apart.  In a dense system that is 8 consecutive particles of a row (they
-// span about one cell width); where a species is sparse or clustered the table cuts chunks short instead, which
-// keeps the bounding box tight (few wasted candidates) and the frame coordinates small (FP32 ulp of a
-// displacement <= 1e-6 fm).  The frame's origin cell is the middle of the chunk's extent.
+// Both passes of one chunk.  The chunk table (k1_cells.cu) makes every chunk COMPACT: up to 8 same-species targets
+// from a few neighbouring cells, at most ~16-20 fm apart.  In a dense system that is 8 consecutive particles of a
+// row (they span about one cell width); where a species is sparse or clustered the table groups the particles of
+// a small block of cells instead.  Compact chunks keep the bounding box tight (few wasted candidates) and the
+// frame coordinates small (FP32 ulp of a displacement <= 1e-6 fm).  The frame's origin cell is the middle of the
+// targets' cell range.
 template <bool CUT, bool ENERGY, bool STATS>
 __device__ __forceinline__ void chunk_passes(const ChunkArgs& A, const PairConsts& c, WarpShared& sh, const int lane,
                                              const int pr, const SpeciesGrid& gt, const int st_sp, const bool chunk_p,
-                                             const float4 tp, const int tc, const int nvalid, Accum& acc,
+                                             const float4 tp, const int tc, const unsigned active, Accum& acc,
                                              unsigned long long* st) {
-  const int c_first = __shfl_sync(0xffffffffu, tc, 0), c_last = __shfl_sync(0xffffffffu, tc, nvalid - 1);
-  const int oy = PASTA_CY(c_first), oz = PASTA_CZ(c_first);
-  const int ox = PASTA_CX(c_first) + (PASTA_CX(c_last) - PASTA_CX(c_first)) / 2;  // sorted by cx within the row
-  const int mx = PASTA_CX(tc) - ox, my = 0, mz = 0;
-  const bool mine = lane < nvalid;
-  const unsigned active = nvalid >= 32 ? 0xffffffffu : ((1u << nvalid) - 1u);
+  const bool mine = ((active >> lane) & 1u) != 0;
   const int j0 = 0;
+  // cell offsets from target 0's cell in the nearest periodic image, then the middle of their range as origin
+  const int c0 = __shfl_sync(0xffffffffu, tc, 0);
+  int mx = min_image_cells(PASTA_CX(tc) - PASTA_CX(c0), gt.ncx);
+  int my = min_image_cells(PASTA_CY(tc) - PASTA_CY(c0), gt.ncell);
+  int mz = min_image_cells(PASTA_CZ(tc) - PASTA_CZ(c0), gt.ncell);
+  int lo_x = mine ? mx : 0, hi_x = lo_x, lo_y = mine ? my : 0, hi_y = lo_y, lo_z = mine ? mz : 0, hi_z = lo_z;
+#pragma unroll
+  for (int o = 1; o < T; o <<= 1) {  // targets sit in lanes [0, T)
+    lo_x = min(lo_x, __shfl_xor_sync(0xffffffffu, lo_x, o)); hi_x = max(hi_x, __shfl_xor_sync(0xffffffffu, hi_x, o));
+    lo_y = min(lo_y, __shfl_xor_sync(0xffffffffu, lo_y, o)); hi_y = max(hi_y, __shfl_xor_sync(0xffffffffu, hi_y, o));
+    lo_z = min(lo_z, __shfl_xor_sync(0xffffffffu, lo_z, o)); hi_z = max(hi_z, __shfl_xor_sync(0xffffffffu, hi_z, o));
+  }
+  const int sx = __shfl_sync(0xffffffffu, (lo_x + hi_x) >> 1, 0), sy = __shfl_sync(0xffffffffu, (lo_y + hi_y) >> 1, 0),
+            sz = __shfl_sync(0xffffffffu, (lo_z + hi_z) >> 1, 0);
+  mx -= sx; my -= sy; mz -= sz;
+  int ox = (PASTA_CX(c0) + sx) % gt.ncx, oy = (PASTA_CY(c0) + sy) % gt.ncell, oz = (PASTA_CZ(c0) + sz) % gt.ncell;
+  ox += ox < 0 ? gt.ncx : 0;
+  oy += oy < 0 ? gt.ncell : 0;
+  oz += oz < 0 ? gt.ncell : 0;
   // ---- pass 0: proton sources, pass 1: neutron sources -------------------------------------------------
 #pragma unroll
   for (int sp = 0; sp < 2; ++sp) {
@@ -427,27 +442,30 @@ __global__ void __launch_bounds__(WARPS * 32, K2_MINB) k2_chunk_kernel(const Chu
   // everything derived from it) in uniform registers, off the vector register file
   const int wib = __reduce_or_sync(0xffffffffu, (int)(threadIdx.x >> 5));
   const int pr = lane / NPH, ph = lane % NPH;  // this lane's target pair and phase
-  const int chunk = blockIdx.x * WARPS + wib;
-  if (chunk >= A.nprim + A.counts[0]) return;  // the launch covers an upper bound of the number of chunks
+  // overflow entries first (odd-sized chunks: better at the start of the launch than in its tail), then the
+  // primary ones in slot order; the launch covers an upper bound of the number of chunks
+  const int widx = blockIdx.x * WARPS + wib, n_over = A.counts[0];
+  if (widx >= A.nprim + n_over) return;
+  const int chunk = widx < n_over ? A.nprim + widx : widx - n_over;
   WarpShared& sh = shared[wib];
 
-  const int entry = __ldg(A.chunk_tab + chunk);
-  const int base = entry & 0x3ffffff, nvalid = entry >> 26;
-  if (nvalid == 0) return;  // empty primary entry
-  const bool chunk_p = base < A.Np;
+  // ---- targets: lane l < 8 holds the chunk's l-th target (valid ones come first) -----------------------------
+  const int slot = lane < T ? __ldg(A.chunk_tab + (int64_t)chunk * T + lane) : -1;
+  const unsigned active = __ballot_sync(0xffffffffu, slot >= 0);
+  if (active == 0) return;  // empty primary entry
+  const int slot0 = __shfl_sync(0xffffffffu, slot, 0);
+  const bool chunk_p = slot0 < A.Np;
   const int st_sp = chunk_p ? 0 : 1;
   const SpeciesGrid& gt = A.g[st_sp];
-
-  // ---- targets: lane l < nvalid holds target l ------------------------------------------------------------
-  const int tl = lane < nvalid ? lane : 0;
-  const float4 tp = __ldg(A.pos4 + base + tl);
-  const int tc = __ldg(A.cxyz + base + tl);
+  const int tslot = slot >= 0 ? slot : slot0;
+  const float4 tp = __ldg(A.pos4 + tslot);
+  const int tc = __ldg(A.cxyz + tslot);
 
   Accum acc;
   acc.fx = acc.fy = acc.fz = acc.e = acc.s1 = acc.s2 = make_float2(0.f, 0.f);
   unsigned long long st[3] = {0, 0, 0};
 
-  chunk_passes<CUT, ENERGY, STATS>(A, c, sh, lane, pr, gt, st_sp, chunk_p, tp, tc, nvalid, acc, st);
+  chunk_passes<CUT, ENERGY, STATS>(A, c, sh, lane, pr, gt, st_sp, chunk_p, tp, tc, active, acc, st);
 
   // ---- combine the phases' FP32 partials in FP64 ------------------------------------------------------------
   // quantity index q = 4 * (target within the pair) + {fx, fy, fz, e}; a transposing butterfly over the
@@ -477,18 +495,17 @@ __global__ void __launch_bounds__(WARPS * 32, K2_MINB) k2_chunk_kernel(const Chu
     qbase += upper ? half : 0;
     nq = half;
   }
-  if (ph < L8) {
 #pragma unroll
-    for (int j = 0; j < 8 / L8; ++j) {
-      const int q = qbase + j, tgt = 2 * pr + (q >> 2), comp = q & 3;
-      if (tgt < nvalid) {
-        const int i = __ldg(A.perm + base + tgt);
-        if (comp < 3) {
-          A.F[3 * (int64_t)i + comp] = -v[j];  // d was x_j - x_i
-        } else if (ENERGY) {
-          // every target met itself once in its own species' pass at r = 0: remove V(0) = a + b + c
-          A.e[i] = 0.5 * (v[j] - (double)c.v_self);
-        }
+  for (int j = 0; j < 8 / L8; ++j) {
+    const int q = qbase + j, tgt = 2 * pr + (q >> 2), comp = q & 3;
+    const int tgt_slot = __shfl_sync(0xffffffffu, slot, tgt);
+    if (ph < L8 && tgt_slot >= 0) {
+      const int i = __ldg(A.perm + tgt_slot);
+      if (comp < 3) {
+        A.F[3 * (int64_t)i + comp] = -v[j];  // d was x_j - x_i
+      } else if (ENERGY) {
+        // every target met itself once in its own species' pass at r = 0: remove V(0) = a + b + c
+        A.e[i] = 0.5 * (v[j] - (double)c.v_self);
       }
     }
   }
@@ -513,7 +530,7 @@ int k2_chunk_forces(Sim* s, bool with_energy, bool stats) {
   A.Np = (int32_t)s->Np;
   A.chunk_tab = s->chunk_tab.as<int32_t>();
   A.counts = s->counters.as<int32_t>() + 2 * 24;
-  A.nprim = (int32_t)((s->N + T - 1) / T);
+  A.nprim = (int32_t)s->chunk_nprim;
   for (int sp = 0; sp < 2; ++sp) {
     const Grid& g = s->grid_sp[sp];
     A.g[sp].ncell = g.ncell;

@@ -113,7 +113,8 @@ struct Sim {
   // [max_chunks, 2 max_chunks) the list of chunks that need several rounds; the counters live in
   // counters[24] (int32 view [48]: number of chunks, [49]: length of that list)
   Buffer chunk_tab;
-  int64_t max_chunks = 0;
+  int64_t max_chunks = 0;   // launch bound of the pair kernel: chunk_nprim primary entries + overflow capacity
+  int64_t chunk_nprim = 0;
 
   // timing: pairs of events (start, stop) tagged with the kernel group they bracket
   bool timing = false;

@@ -357,3 +357,35 @@ def test_exact_zero_skipping_changes_nothing_that_matters(orc, N, density, r_c, 
         nz = inr & (pp | (r2 * (math.log2(math.e) / 2.5) < 126.0))
         assert abs(nonzero - int(nz.sum())) <= 4
     assert nonzero <= pairs
+
+
+@pytest.mark.parametrize("cfg,nsteps,nsample", [(3, 10000, 4096), (3, 20000, 4096), (5, 6000, 1024)])
+def test_evolved_clustered_state_snapshots(orc, cfg, nsteps, nsample):
+    """Snapshot parity during the decompression runs (long configs are never run on the oracle; the
+    state is read back and forces, PE, cells and labels are compared on identical positions).  The evolved states
+    are clustered (dense fragments in a neutron gas): pair forces of ~50 MeV/fm cancel to a few MeV/fm, the
+    regime in which the FP32 coordinate quantum matters most; both gates of D17 must hold here too."""
+    c = inputs.CONFIGS[cfg]
+    p = pasta.default_params(r_c=c["r_c"], thermostat_interval=c["thermostat_interval"],
+                             scale_per_step=c["scale_per_step"])
+    with pasta.Sim(c["N"], c["Y_P"], c["density"], c["T"], params=p, seed=1) as sim:
+        sim.step(nsteps, c["dt"])
+        x, v, is_p, L, step = sim.get_state()
+        assert step == nsteps and L == pytest.approx(inputs.box_length(c["N"], c["density"]) * c["scale_per_step"] ** nsteps,
+                                                     rel=1e-11)
+        x, is_p = _np(x), _np(is_p)
+        F, pe = sim.forces()
+        F, e = _np(F), _np(sim.particle_energies())
+        t = np.sort(np.random.default_rng(cfg).choice(c["N"], size=nsample, replace=False))
+        Fo, eo, _, _ = orc.forces(x, is_p, L, _oparams(orc, p), targets=t)
+        _check_forces(F[t], Fo)
+        assert abs(e[t].sum() - eo.sum()) <= 3 * PE_TOL * abs(eo.sum())
+        ke, _ = sim.energy()
+        assert ke == pytest.approx(1.5 * c["N"] * c["T"], rel=1e-9)        # rescaled every 10 steps (D7, D8)
+        cid, start, nc = sim.cells()
+        cid_o, start_o = orc.cells(x, L, nc)
+        assert np.array_equal(_np(cid), cid_o) and np.array_equal(_np(start), start_o)
+        if c["N"] <= 60000:
+            label, n = sim.clusters(c["r_cl"])
+            lo, _, _, no = orc.clusters(x, is_p, L, c["r_cl"])
+            assert n == no and np.array_equal(_np(label), lo)
