@@ -33,30 +33,11 @@ Grid make_grid(double L, double r_c, int32_t k, int32_t xsub) {
   return g;
 }
 
-// c = min(ncell-1, floor(x * inv_w)) -- a single correctly rounded FP64 multiply, then floor (D14).
-__device__ __forceinline__ int cell_coord(double x, double inv_w, int ncell) {
-  int q = (int)floor(__dmul_rn(x, inv_w));
-  q = q > ncell - 1 ? ncell - 1 : q;
-  return q < 0 ? 0 : q;
-}
-
-struct GridPair {
-  int ncell[2], ncx[2];
-  int base[2];  // first bin of the species' grid: base[0] = 0, base[1] = number of cells of grid 0
-  double inv_w[2], w[2], inv_wx[2], wx[2];
-};
-
 __global__ void k1_count_kernel(int64_t N, const double* __restrict__ x, const uint8_t* __restrict__ is_p,
                                 const GridPair g, int32_t* __restrict__ pbin, int32_t* __restrict__ bin_count) {
   int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= N) return;
-  const int sp = is_p[i] ? 0 : 1;
-  const int nc = g.ncell[sp], ncx = g.ncx[sp];
-  const double iw = g.inv_w[sp];
-  int cx = cell_coord(x[3 * i + 0], g.inv_wx[sp], ncx);
-  int cy = cell_coord(x[3 * i + 1], iw, nc);
-  int cz = cell_coord(x[3 * i + 2], iw, nc);
-  const int bin = g.base[sp] + (cz * nc + cy) * ncx + cx;
+  const int bin = force_bin(g, is_p[i] ? 0 : 1, x[3 * i + 0], x[3 * i + 1], x[3 * i + 2]);
   pbin[i] = bin;
   atomicAdd(&bin_count[bin], 1);
 }
@@ -122,28 +103,26 @@ __global__ void __launch_bounds__(SCAN_T) scan_local_kernel(const int32_t* __res
   if (threadIdx.x == 0) block_sums[blockIdx.x] = total;
 }
 
-__global__ void __launch_bounds__(SCAN_T) scan_top_kernel(int32_t* __restrict__ block_sums, int nb,
-                                                          int32_t* __restrict__ out_total) {
-  __shared__ int carry_s;
-  if (threadIdx.x == 0) carry_s = 0;
-  __syncthreads();
-  for (int base = 0; base < nb; base += SCAN_T) {
-    int idx = base + threadIdx.x;
-    int v = idx < nb ? block_sums[idx] : 0;
-    int total;
-    int ex = block_exclusive_scan(v, &total);
-    int carry = carry_s;
-    if (idx < nb) block_sums[idx] = carry + ex;
-    __syncthreads();
-    if (threadIdx.x == 0) carry_s = carry + total;
-    __syncthreads();
-  }
-  if (threadIdx.x == 0) *out_total = carry_s;
-}
-
+// Second (and last) launch of the scan: every block sums the totals of the blocks before it (a few hundred
+// numbers), adds that to its tile; the last block also writes the grand total to out[n].
 __global__ void __launch_bounds__(SCAN_T) scan_add_kernel(int32_t* __restrict__ out, int64_t n,
                                                           const int32_t* __restrict__ block_sums) {
-  const int add = block_sums[blockIdx.x];
+  __shared__ int ws[SCAN_T / 32];
+  __shared__ int add_s;
+  int part = 0;
+  for (int k = threadIdx.x; k < (int)blockIdx.x; k += SCAN_T) part += block_sums[k];
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) part += __shfl_xor_sync(0xffffffffu, part, o);
+  if ((threadIdx.x & 31) == 0) ws[threadIdx.x >> 5] = part;
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    int a = 0;
+    for (int k = 0; k < SCAN_T / 32; ++k) a += ws[k];
+    add_s = a;
+    if (blockIdx.x == gridDim.x - 1) out[n] = a + block_sums[blockIdx.x];
+  }
+  __syncthreads();
+  const int add = add_s;
   const int64_t base = (int64_t)blockIdx.x * SCAN_TILE + (int64_t)threadIdx.x * SCAN_ITEMS;
 #pragma unroll
   for (int k = 0; k < SCAN_ITEMS; ++k)
@@ -155,9 +134,8 @@ int scan_exclusive(Sim* s, const int32_t* in, int32_t* out, int64_t n) {
   PASTA_TRY(buffer_reserve(s, &s->scan_tmp, sizeof(int32_t) * (size_t)(nb + 1)));
   int32_t* tmp = s->scan_tmp.as<int32_t>();
   scan_local_kernel<<<nb, SCAN_T, 0, s->stream>>>(in, out, n, tmp);
-  scan_top_kernel<<<1, SCAN_T, 0, s->stream>>>(tmp, nb, out + n);
   scan_add_kernel<<<nb, SCAN_T, 0, s->stream>>>(out, n, tmp);
-  s->launches += 3;
+  s->launches += 2;
   PASTA_CUDA_OK(cudaGetLastError());
   return PASTA_OK;
 }
@@ -187,13 +165,36 @@ __global__ void k1_order_kernel(int64_t nbins, const int32_t* __restrict__ bin_s
   }
 }
 
+// Sorted slot t -> its particle, positions relative to the cell centre, packed cell coordinates.
+// FUSED_ORDER: `perm_in` holds the members of every bin in the arrival order of the scatter's atomics; slot t
+// takes the member of its bin with exactly (t - first slot of the bin) smaller indices, so the sorted order
+// (and with it the summation order of the force kernel) is ascending in the original index whatever the
+// arrival order was, and writes it to `perm_out`.  (Thin-cell bins hold a particle or two; the uniform one-grid
+// variant, whose bins hold hundreds, orders them with k1_order_kernel instead.)
+template <bool FUSED_ORDER>
 __global__ void k1_gather_kernel(int64_t N, const double* __restrict__ x, const int32_t* __restrict__ pbin,
-                                 const int32_t* __restrict__ perm, const GridPair g, double sigma,
-                                 float4* __restrict__ pos4, int32_t* __restrict__ cxyz) {
+                                 const int32_t* __restrict__ perm_in, int32_t* __restrict__ perm_out,
+                                 const int32_t* __restrict__ bin_start, const GridPair g, double sigma,
+                                 float4* __restrict__ pos4, int32_t* __restrict__ cxyz,
+                                 int32_t* __restrict__ zero_me) {
   int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (t == 0 && zero_me) *zero_me = 0;  // the overflow counter of the chunk table
   if (t >= N) return;
-  const int i = perm[t];
+  int i = perm_in[t];
   const int bin = pbin[i];
+  if (FUSED_ORDER) {
+    const int lo = bin_start[bin], hi = bin_start[bin + 1];
+    if (hi - lo > 1) {
+      const int want = (int)t - lo;
+      for (int a = lo; a < hi; ++a) {
+        const int ia = perm_in[a];
+        int rank = 0;
+        for (int b = lo; b < hi; ++b) rank += perm_in[b] < ia ? 1 : 0;
+        if (rank == want) i = ia;
+      }
+    }
+    perm_out[t] = i;
+  }
   const int sp = bin >= g.base[1] ? 1 : 0;
   const int id = bin - g.base[sp], nc = g.ncell[sp], ncx = g.ncx[sp];
   const double w = g.w[sp];
@@ -346,7 +347,9 @@ static int auto_xsub(double L, double r_c, int k, int64_t n_species) {
   return xsub;
 }
 
-int k1_build(Sim* s, bool uniform_grid) {
+// Grids of the two species for the current box, buffers, and a zeroed histogram.  (The scatter kernel counts the
+// histogram back down to zero, so the memset is needed only when the table grows or somebody else used it.)
+int k1_setup(Sim* s, bool uniform_grid, GridPair* gp) {
   const int64_t N = s->N;
   // the reference kernel and the pair counter walk ONE isotropic grid; the chunk kernel takes a grid per
   // species, each cell sliced into thin cells along x (rows sorted in x: tight source ranges, compact chunks)
@@ -358,7 +361,7 @@ int k1_build(Sim* s, bool uniform_grid) {
   const int xs1 = uniform ? 1 : (s->prm.x_subdiv > 0 ? s->prm.x_subdiv : auto_xsub(s->L, s->prm.r_c, k1, N - s->Np));
   s->grid_sp[0] = make_grid(s->L, s->prm.r_c, k0, xs0);
   s->grid_sp[1] = make_grid(s->L, s->prm.r_c, k1, xs1);
-  GridPair g;
+  GridPair& g = *gp;
   for (int sp = 0; sp < 2; ++sp) {
     g.ncell[sp] = s->grid_sp[sp].ncell;
     g.ncx[sp] = s->grid_sp[sp].ncx;
@@ -372,23 +375,55 @@ int k1_build(Sim* s, bool uniform_grid) {
   s->bin_base[0] = 0;
   s->bin_base[1] = s->grid_sp[0].nc3;
   const int64_t nbins = s->grid_sp[0].nc3 + s->grid_sp[1].nc3;
+  const void* before = s->bin_count.ptr;
   PASTA_TRY(buffer_reserve(s, &s->bin_count, sizeof(int32_t) * (size_t)(nbins + 1)));
   PASTA_TRY(buffer_reserve(s, &s->bin_start, sizeof(int32_t) * (size_t)(nbins + 1)));
+  PASTA_TRY(buffer_reserve(s, &s->perm_raw, sizeof(int32_t) * (size_t)N));
+  if (s->bin_count.ptr != before) s->bins_zeroed = 0;
+  if (s->bins_zeroed < nbins + 1) {
+    PASTA_CUDA_OK(cudaMemsetAsync(s->bin_count.ptr, 0, s->bin_count.bytes, s->stream));
+    s->bins_zeroed = (int64_t)(s->bin_count.bytes / sizeof(int32_t));
+  }
+  return PASTA_OK;
+}
+
+int k1_build(Sim* s, bool uniform_grid) {
+  const int64_t N = s->N;
+  const bool uniform = uniform_grid || s->prm.force_variant == 1;
+  GridPair g;
+  const int B = 256;
+  if (!(s->hist_valid && s->hist_uniform == uniform)) {
+    if (s->hist_valid) s->bins_zeroed = 0;  // a histogram for the other kind of grid is sitting in the table
+    PASTA_TRY(k1_setup(s, uniform_grid, &g));
+    k1_count_kernel<<<grid_for(N, B), B, 0, s->stream>>>(N, s->x.as<double>(), s->is_p.as<uint8_t>(), g,
+                                                         s->cell_id.as<int32_t>(), s->bin_count.as<int32_t>());
+    s->launches += 1;
+  } else {
+    PASTA_TRY(k1_setup(s, uniform_grid, &g));  // same L, same grids: recomputes g, allocates and zeroes nothing
+  }
+  s->hist_valid = false;
+  const int64_t nbins = s->grid_sp[0].nc3 + s->grid_sp[1].nc3;
   int32_t* cnt = s->bin_count.as<int32_t>();
   int32_t* start = s->bin_start.as<int32_t>();
-  PASTA_CUDA_OK(cudaMemsetAsync(cnt, 0, sizeof(int32_t) * (size_t)(nbins + 1), s->stream));
-  const int B = 256;
-  k1_count_kernel<<<grid_for(N, B), B, 0, s->stream>>>(N, s->x.as<double>(), s->is_p.as<uint8_t>(), g,
-                                                       s->cell_id.as<int32_t>(), cnt);
-  s->launches += 1;
   PASTA_TRY(scan_exclusive(s, cnt, start, nbins));
-  k1_scatter_kernel<<<grid_for(N, B), B, 0, s->stream>>>(N, s->cell_id.as<int32_t>(), start, cnt, s->perm.as<int32_t>());
-  k1_order_kernel<<<grid_for(nbins, B), B, 0, s->stream>>>(nbins, start, s->perm.as<int32_t>());
   const double sigma = sqrt(1.4426950408889634074 / (2.0 * s->prm.Lambda));
-  k1_gather_kernel<<<grid_for(N, B), B, 0, s->stream>>>(N, s->x.as<double>(), s->cell_id.as<int32_t>(),
-                                                        s->perm.as<int32_t>(), g, sigma, s->pos4.as<float4>(),
-                                                        s->cxyz.as<int32_t>());
-  s->launches += 3;
+  int32_t* n_overflow = s->counters.as<int32_t>() + 2 * 24;
+  if (uniform) {
+    k1_scatter_kernel<<<grid_for(N, B), B, 0, s->stream>>>(N, s->cell_id.as<int32_t>(), start, cnt, s->perm.as<int32_t>());
+    k1_order_kernel<<<grid_for(nbins, B), B, 0, s->stream>>>(nbins, start, s->perm.as<int32_t>());
+    k1_gather_kernel<false><<<grid_for(N, B), B, 0, s->stream>>>(N, s->x.as<double>(), s->cell_id.as<int32_t>(),
+                                                                 s->perm.as<int32_t>(), nullptr, start, g, sigma,
+                                                                 s->pos4.as<float4>(), s->cxyz.as<int32_t>(), nullptr);
+    s->launches += 3;
+  } else {
+    k1_scatter_kernel<<<grid_for(N, B), B, 0, s->stream>>>(N, s->cell_id.as<int32_t>(), start, cnt,
+                                                           s->perm_raw.as<int32_t>());
+    k1_gather_kernel<true><<<grid_for(N, B), B, 0, s->stream>>>(N, s->x.as<double>(), s->cell_id.as<int32_t>(),
+                                                                s->perm_raw.as<int32_t>(), s->perm.as<int32_t>(), start,
+                                                                g, sigma, s->pos4.as<float4>(), s->cxyz.as<int32_t>(),
+                                                                n_overflow);
+    s->launches += 2;
+  }
   if (!uniform) {
     // builder per species (DENSE row runs: at least 3 particles per cell on average), the extent limit of a row
     // run (three cell widths, at most 16 fm) and the capacity of the table: a bound on the number of chunks
@@ -425,8 +460,6 @@ int k1_build(Sim* s, bool uniform_grid) {
     s->chunk_nprim = cg.nprim;
     s->max_chunks = cg.nprim + overflow;
     PASTA_TRY(buffer_reserve(s, &s->chunk_tab, sizeof(int32_t) * CHUNK_T * (size_t)(s->max_chunks + 8)));
-    int32_t* n_overflow = s->counters.as<int32_t>() + 2 * 24;
-    PASTA_CUDA_OK(cudaMemsetAsync(n_overflow, 0, sizeof(int32_t), s->stream));
     if (any_rows) {
       k1_chunk_rows_kernel<<<grid_for(cg.nprim, 128), 128, 0, s->stream>>>(
           (int32_t)N, (int32_t)s->Np, s->cxyz.as<int32_t>(), start, g, cg, s->chunk_tab.as<int32_t>(), n_overflow);
@@ -448,6 +481,8 @@ int k1_build(Sim* s, bool uniform_grid) {
 // force evaluation rebuilds them anyway).
 int k1_export_cells(Sim* s, int32_t* cell_id_dev, int32_t* cell_start_dev) {
   const Grid g = make_grid(s->L, s->prm.r_c, s->prm.cell_subdiv);
+  s->hist_valid = false;  // cell_id and the histogram table are about to hold the exported grid
+  s->bins_zeroed = 0;
   PASTA_TRY(buffer_reserve(s, &s->bin_count, sizeof(int32_t) * (size_t)(g.nc3 + 1)));
   PASTA_TRY(buffer_reserve(s, &s->bin_start, sizeof(int32_t) * (size_t)(g.nc3 + 1)));
   int32_t* cnt = s->bin_count.as<int32_t>();

@@ -14,15 +14,26 @@ __device__ __forceinline__ double wrap_coord(double x, double L, double invL) {
   return w;
 }
 
-// First half kick, drift, scale and wrap (O2 steps 1-2):  v += h F;  x = wrap(s (x + dt v)).
-__global__ void k3_kick_drift_kernel(int64_t n3, double* __restrict__ x, double* __restrict__ v,
-                                     const double* __restrict__ F, double h, double dt, double scale, double L,
-                                     double invL) {
-  int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-  if (k >= n3) return;
-  const double vk = v[k] + h * F[k];
-  v[k] = vk;
-  x[k] = wrap_coord(scale * (x[k] + dt * vk), L, invL);
+// First half kick, drift, scale and wrap (O2 steps 1-2):  v += h F;  x = wrap(s (x + dt v)) -- and, fused with it,
+// the first step of the cell list of the new positions (K1 a1): the particle's (species, cell) bin on its
+// species' force grid and the histogram of the bins.  One thread per particle.
+__global__ void k3_kick_drift_count_kernel(int64_t N, double* __restrict__ x, double* __restrict__ v,
+                                           const double* __restrict__ F, const uint8_t* __restrict__ is_p, double h,
+                                           double dt, double scale, double L, double invL, const GridPair g,
+                                           int32_t* __restrict__ pbin, int32_t* __restrict__ bin_count) {
+  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= N) return;
+  double xn[3];
+#pragma unroll
+  for (int k = 0; k < 3; ++k) {
+    const double vk = v[3 * i + k] + h * F[3 * i + k];
+    v[3 * i + k] = vk;
+    xn[k] = wrap_coord(scale * (x[3 * i + k] + dt * vk), L, invL);
+    x[3 * i + k] = xn[k];
+  }
+  const int bin = force_bin(g, is_p[i] ? 0 : 1, xn[0], xn[1], xn[2]);
+  pbin[i] = bin;
+  atomicAdd(&bin_count[bin], 1);
 }
 
 constexpr int RED_T = 256;
@@ -99,12 +110,16 @@ static int red_blocks(int64_t n) {
   return (int)(b < 1 ? 1 : (b > 1184 ? 1184 : b));  // 148 SMs x 8 resident blocks
 }
 
-int k3_kick_drift(Sim* s, double dt, double scale, double L_new) {
-  const int64_t n3 = 3 * s->N;
-  k3_kick_drift_kernel<<<grid_for(n3, 256), 256, 0, s->stream>>>(n3, s->x.as<double>(), s->v.as<double>(),
-                                                                 s->F.as<double>(), dt / (2.0 * s->prm.mass), dt, scale,
-                                                                 L_new, 1.0 / L_new);
+// The caller has set s->L to the box of the NEW positions.
+int k3_kick_drift_count(Sim* s, double dt, double scale) {
+  GridPair g;
+  PASTA_TRY(k1_setup(s, false, &g));
+  k3_kick_drift_count_kernel<<<grid_for(s->N, 128), 128, 0, s->stream>>>(
+      s->N, s->x.as<double>(), s->v.as<double>(), s->F.as<double>(), s->is_p.as<uint8_t>(), dt / (2.0 * s->prm.mass),
+      dt, scale, s->L, 1.0 / s->L, g, s->cell_id.as<int32_t>(), s->bin_count.as<int32_t>());
   s->launches += 1;
+  s->hist_valid = true;
+  s->hist_uniform = s->prm.force_variant == 1;
   PASTA_CUDA_OK(cudaGetLastError());
   return PASTA_OK;
 }
@@ -128,6 +143,7 @@ int k3_kick_ke(Sim* s, double dt, bool rescale) {
 
 int k3_wrap_scale(Sim* s, double scale, double L_new) {
   const int64_t n3 = 3 * s->N;
+  s->hist_valid = false;
   k3_wrap_scale_kernel<<<grid_for(n3, 256), 256, 0, s->stream>>>(n3, s->x.as<double>(), scale, L_new, 1.0 / L_new);
   s->launches += 1;
   PASTA_CUDA_OK(cudaGetLastError());

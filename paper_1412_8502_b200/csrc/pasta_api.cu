@@ -55,7 +55,7 @@ void buffer_release(Sim* s, Buffer* b) {
 
 static void release_all(Sim* s) {
   Buffer* bs[] = {&s->x, &s->v, &s->F, &s->e, &s->is_p, &s->cell_id, &s->bin_count, &s->bin_start, &s->scan_tmp,
-                  &s->perm, &s->pos4, &s->cxyz, &s->partials, &s->scalars, &s->counters, &s->cl_parent, &s->cl_A,
+                  &s->perm, &s->perm_raw, &s->pos4, &s->cxyz, &s->partials, &s->scalars, &s->counters, &s->cl_parent, &s->cl_A,
                   &s->cl_Z, &s->cl_cell_id, &s->cl_count, &s->cl_start, &s->cl_perm, &s->chunk_tab};
   for (Buffer* b : bs) buffer_release(s, b);
 }
@@ -288,11 +288,11 @@ int pasta_step(pasta_sim* sim, int64_t n, double dt) {
       set_error("pasta_step: box side %g would fall below 2 r_c", L_new);
       return PASTA_EINVAL;
     }
+    s->L = L_new;
     {
       Timer t(s, 2);
-      PASTA_TRY(k3_kick_drift(s, dt, sc, L_new));
+      PASTA_TRY(k3_kick_drift_count(s, dt, sc));
     }
-    s->L = L_new;
     s->clusters_valid = false;
     PASTA_TRY(evaluate_forces(s, energy));
     s->step_count += 1;

@@ -54,6 +54,28 @@ Grid make_grid(double L, double r_c, int32_t k, int32_t xsub = 1);
 #define PASTA_CY(c) (((c) >> 12) & 1023)
 #define PASTA_CZ(c) (((c) >> 22) & 1023)
 
+// The two species' grids as the K1 kernels (and the fused kick-drift-count kernel of K3) see them.
+struct GridPair {
+  int ncell[2], ncx[2];
+  int base[2];  // first bin of the species' grid: base[0] = 0, base[1] = number of cells of grid 0
+  double inv_w[2], w[2], inv_wx[2], wx[2];
+};
+
+#ifdef __CUDACC__
+// c = min(ncell-1, floor(x * inv_w)) -- a single correctly rounded FP64 multiply, then floor (D14).
+__device__ __forceinline__ int cell_coord(double x, double inv_w, int ncell) {
+  int q = (int)floor(__dmul_rn(x, inv_w));
+  q = q > ncell - 1 ? ncell - 1 : q;
+  return q < 0 ? 0 : q;
+}
+// (species, cell) bin of a particle on its species' force grid
+__device__ __forceinline__ int force_bin(const GridPair& g, int sp, double x, double y, double z) {
+  const int nc = g.ncell[sp], ncx = g.ncx[sp];
+  const int cx = cell_coord(x, g.inv_wx[sp], ncx), cy = cell_coord(y, g.inv_w[sp], nc), cz = cell_coord(z, g.inv_w[sp], nc);
+  return g.base[sp] + (cz * nc + cy) * ncx + cx;
+}
+#endif
+
 // Constants of the FP32 pair arithmetic, derived on the host in FP64 (k2_force.cu explains them).
 struct PairConsts {
   float sigma;       // coordinate pre-scale sqrt(log2(e) / (2 Lambda))
@@ -84,6 +106,9 @@ struct Sim {
   bool forces_valid = false;
   bool energies_valid = false;
   bool clusters_valid = false;
+  bool hist_valid = false;    // bin_count/cell_id hold the histogram of the current x on the current force grids
+  bool hist_uniform = false;  // ... built for the uniform (one grid) variant
+  int64_t bins_zeroed = 0;    // bin_count[0, bins_zeroed) is known to be all zero (the scatter leaves it so)
   int64_t launches = 0;
 
   // state (device)
@@ -96,6 +121,7 @@ struct Sim {
   Buffer bin_count;   // int32[2 nc3 + 1] scratch histogram over (species, cell) bins
   Buffer bin_start;   // int32[2 nc3 + 1] exclusive scan; protons' bins first
   Buffer scan_tmp;    // block sums of the scan
+  Buffer perm_raw;    // int32[N]   sorted slot -> original index, members of a bin in arrival order
   Buffer perm;        // int32[N]   sorted slot -> original index
   Buffer pos4;        // float4[N]  sorted: sigma * cell-relative position, .w = cell x index
   Buffer cxyz;        // int32[N]   sorted: packed cell coordinates (cx | cy<<10 | cz<<20)
@@ -127,7 +153,9 @@ struct Sim {
 
 // ---- kernel launchers (one translation unit each) ---------------------------------------------------
 // K1  k1_cells.cu
-int k1_build(Sim* s, bool uniform_grid = false);                                // cell ids, (species,cell) counting sort, pos4/perm
+int k1_setup(Sim* s, bool uniform_grid, GridPair* g);  // grids for the current L, buffers, a zeroed histogram
+int k1_build(Sim* s, bool uniform_grid = false);       // (species,cell) counting sort, pos4/perm, chunk table; uses the
+                                                       // histogram of k3_kick_drift_count if s->hist_valid
 int k1_export_cells(Sim* s, int32_t* cell_id_dev, int32_t* cell_start_dev);
 int scan_exclusive(Sim* s, const int32_t* in, int32_t* out, int64_t n);  // out[0..n] (n+1 entries)
 // K2  k2_force.cu
@@ -137,7 +165,7 @@ int k2_reference_forces(Sim* s, bool with_energy);     // variant 1: thread per 
 int k2_chunk_forces(Sim* s, bool with_energy, bool stats);  // variant 2: chunk kernel (k2_chunk.cu)
 // K3  k3_integrate.cu
 int k3_init_state(Sim* s, uint64_t seed);
-int k3_kick_drift(Sim* s, double dt, double scale, double L_new);
+int k3_kick_drift_count(Sim* s, double dt, double scale);  // kick, drift, scale, wrap for box s->L + cell histogram
 int k3_kick_ke(Sim* s, double dt, bool rescale);       // second half kick + KE (+ rescale)
 int k3_wrap_scale(Sim* s, double scale, double L_new); // x = wrap(scale x)
 int k3_kinetic(Sim* s, double* ke_host);
