@@ -158,9 +158,18 @@ __device__ __forceinline__ void evaluate(const float4 s, const Targets& t, Accum
   acc.fz = __ffma2_rn(g, dz, acc.fz);
 }
 
-__device__ __forceinline__ int floor_div(int a, int b) {  // b > 0
+// floor(a / b), b > 0.  The listing only ever asks with -b <= a < 2 b (reach + box < L), where it is a
+// comparison; the generic integer division (dozens of instructions) is the fallback.
+__device__ __forceinline__ int floor_div(int a, int b) {
+  if (a >= -b && a < 2 * b) return (a < 0 ? -1 : 0) + (a >= b ? 1 : 0);
   const int q = a / b;
   return (a % b < 0) ? q - 1 : q;
+}
+// a mod n in [0, n) for -n <= a < 2 n, generic otherwise
+__device__ __forceinline__ int wrap_cell(int a, int n) {
+  if (a >= -n && a < 2 * n) return a + (a < 0 ? n : 0) - (a >= n ? n : 0);
+  a %= n;
+  return a + (a < 0 ? n : 0);
 }
 
 // Per-lane cursor into the segment list of a pass: the segment holding the lane's current stream position.
@@ -256,6 +265,7 @@ __device__ __forceinline__ void source_pass(const ChunkArgs& A, const PairConsts
   const int my_lo = (int)floorf((b.lo_y - rc) * gs.inv_wS + 0.5f), my_hi = (int)floorf((b.hi_y + rc) * gs.inv_wS + 0.5f);
   const int mz_lo = (int)floorf((b.lo_z - rc) * gs.inv_wS + 0.5f), mz_hi = (int)floorf((b.hi_z + rc) * gs.inv_wS + 0.5f);
   const int ny = my_hi - my_lo + 1, nrows = ny * (mz_hi - mz_lo + 1);
+  const float inv_ny = 1.0f / (float)ny;
   const int nc = gs.ncell, ncx = gs.ncx;
   const unsigned lt_mask = (1u << lane) - 1u;
 
@@ -270,7 +280,8 @@ __device__ __forceinline__ void source_pass(const ChunkArgs& A, const PairConsts
         const int r = rbase + lane;
         nseg = 0;
         if (r < nrows) {
-          const int my = my_lo + r % ny, mz = mz_lo + r / ny;
+          const int rq = (int)(((float)r + 0.5f) * inv_ny);  // r / ny (ny, r < 2^20: exact)
+          const int my = my_lo + (r - rq * ny), mz = mz_lo + rq;
           yoff = __fmul_rn((float)my, gs.wS);
           zoff = __fmul_rn((float)mz, gs.wS);
           // gap between the row's slab [off - w/2, off + w/2] and the box interval, per axis
@@ -283,9 +294,7 @@ __device__ __forceinline__ void source_pass(const ChunkArgs& A, const PairConsts
             ax_hi = rx + (int)floorf((b.hi_x + xr) * gs.inv_wxS + 0.5f);
             q_lo = floor_div(ax_lo, ncx);
             nseg = floor_div(ax_hi, ncx) - q_lo + 1;
-            int ay = (ry + my) % nc, az = (rz + mz) % nc;
-            ay += ay < 0 ? nc : 0;
-            az += az < 0 ? nc : 0;
+            const int ay = wrap_cell(ry + my, nc), az = wrap_cell(rz + mz, nc);
             rowbase = gs.base + (az * nc + ay) * ncx;
           }
         }
