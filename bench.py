@@ -274,6 +274,11 @@ def run_ours(args, rank, world, local_rank):
             "config": workload_config(args.config, world),
             "pair_interactions_per_s": {"unordered": 0.5 * pairs * steps_per_s, "ordered": pairs * steps_per_s,
                                         "ordered_pairs_per_step": pairs},
+            # K1 and K3 move 76 and 192 algorithmic bytes per particle and step; they are
+            # L2-resident and launch-latency-bound, so these are far below the HBM peak by construction
+            "k1_k3_gbs": {"cells": 76.0 * N / (tm["cells_ms"] / max(1, tm["force_evals"]) * 1e-3) / 1e9,
+                          "integrate": 192.0 * N / (tm["integrate_ms"] / max(1, tm["force_evals"]) * 1e-3) / 1e9,
+                          "hbm_peak": hbm_gbs},
             "kernel_ms": {"cells": tm["cells_ms"] / max(1, tm["force_evals"]), "pair_force": 1e3 * k2_s,
                           "integrate": tm["integrate_ms"] / max(1, tm["force_evals"])},
             "roofline": {
@@ -285,7 +290,11 @@ def run_ours(args, rank, world, local_rank):
                 "ordered_pairs_per_s": pairs / k2_s, "mufu_frac": (pairs * c_mufu / k2_s) / mufu_peak,
                 "peak_source": "%d SMs x %d FP32 lanes x %.0f MHz (sm_max_mhz from %s)" % (
                     SM_COUNT, FP32_LANES_PER_SM, sm_max_mhz, peak_src),
-                "traffic": None,
+                # dram__bytes_read.sum + dram__bytes_write.sum of one K2 launch from the committed ncu --set full
+                # capture (profiles/r1_k2_chunk_v6_ncu.md); config 4 only
+                "traffic": 12.2e6 if args.config == 4 else None, "traffic_unit": "bytes per launch",
+                "frac_at_observed_clock": (achieved / fp32_peak) * sm_max_mhz / clocks["sm_mhz"]
+                if clocks and clocks.get("sm_mhz") else None,
             },
             "e2e": {"value": aggregate_rate(world, e2e_steps, e2e_s), "unit": "steps/s", "h2d_bytes_per_step": 72 * N,
                     "d2h_bytes_per_step": 72 * N, "steps": e2e_steps,
@@ -301,6 +310,57 @@ def run_ours(args, rank, world, local_rank):
         dist.destroy_process_group()
 
 
+def run_sweep(args):
+    """--sweep 3|5: the whole decompression run of BASELINE config 3 or 5 (20 000 steps, n = 0.08 -> 0.00125 fm^-3),
+    timed in chunks of --sweep-chunk steps with CUDA events -- steps/s against density, the axis of the paper's
+    Fig. 1/2 -- then friends-of-friends clustering at r_cl = 3 fm and the composition summary.
+    One JSON line."""
+    import torch
+
+    import paper_1412_8502_b200 as pasta
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the product path has no CPU fallback")
+    c = inputs.CONFIGS[args.sweep]
+    prm = pasta.default_params(r_c=c["r_c"], thermostat_interval=c["thermostat_interval"],
+                               scale_per_step=c["scale_per_step"])
+    sim = pasta.Sim(c["N"], c["Y_P"], c["density"], c["T"], params=prm, seed=1)
+    pts, done = [], 0
+    t_all0 = time.perf_counter()
+    while done < c["steps"]:
+        n = min(args.sweep_chunk, c["steps"] - done)
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record()
+        sim.step(n, c["dt"])
+        b.record()
+        torch.cuda.synchronize()
+        done += n
+        L = sim.box_length()
+        ke, pe = sim.energy()
+        pts.append({"step": done, "L_fm": L, "density": c["N"] / L ** 3, "steps_per_s": 1e3 * n / a.elapsed_time(b),
+                    "PE_per_nucleon": pe / c["N"], "T_kin": ke / (1.5 * c["N"])})
+    wall = time.perf_counter() - t_all0
+    t0 = time.perf_counter()
+    label, ncl = sim.clusters(c["r_cl"])
+    A, Z = sim.cluster_sizes()
+    comp = sim.composition(12)
+    torch.cuda.synchronize()
+    fof_s = time.perf_counter() - t0
+    A = A.cpu().numpy()
+    Z = Z.cpu().numpy()
+    heavy = A >= 12
+    import numpy as np
+
+    hist = {}
+    for a_, z_ in zip(A[heavy].tolist(), Z[heavy].tolist()):
+        hist[(a_ // 20 * 20, z_ // 10 * 10)] = hist.get((a_ // 20 * 20, z_ // 10 * 10), 0) + 1
+    line = {"sweep": args.sweep, "workload": workload_config(args.sweep, 1)["workload"] + ", decompression to 0.00125 fm^-3",
+            "steps": c["steps"], "wall_s": wall, "points": pts, "clusters": ncl, "fof_s": fof_s, "composition": comp,
+            "largest_A": int(A.max()), "AZ_histogram_A20_Z10_bins": {"%d,%d" % k: v for k, v in sorted(hist.items())}}
+    print(json.dumps(line), flush=True)
+    sim.close()
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -312,6 +372,9 @@ def main():
     ap.add_argument("--subdiv", type=int, default=None, help="pasta_params.cell_subdiv override")
     ap.add_argument("--stream-all", action="store_true",
                     help="pasta_params.skip_exact_zeros = 0: stream every candidate out to r_c")
+    ap.add_argument("--sweep", type=int, default=0, choices=[0, 3, 5],
+                    help="run the whole decompression of config 3 or 5 and report steps/s against density")
+    ap.add_argument("--sweep-chunk", type=int, default=1000)
     ap.add_argument("--params", default="", help="comma-separated pasta_params overrides (tuning experiments)")
     ap.add_argument("--cpu-budget", type=float, default=15.0, help="seconds of oracle time for cpu_baseline")
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -319,7 +382,10 @@ def main():
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
-    if args.impl == "reference":
+    if args.sweep:
+        if rank == 0:
+            run_sweep(args)
+    elif args.impl == "reference":
         run_reference(args, rank, world)
     else:
         run_ours(args, rank, world, local_rank)
