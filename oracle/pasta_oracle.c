@@ -30,6 +30,9 @@ typedef struct orc_params {
   double lambda;          /* screening length, fixed to 10 fm */
   double r_c;             /* single cut-off of the BASELINE configs (reading D1) */
   double mass;            /* M = 939 MeV */
+  double r_nuc;           /* the paper's own range split: the nuclear (Gaussian) terms are "assumed
+                             to be zero and not computed" beyond r_nuc = 11.5 fm, independently of the Coulomb
+                             term.  <= 0 (default): no separate nuclear cut-off, every term lives inside r_c (D1) */
 } orc_params;
 
 int orc_num_threads(void) {
@@ -63,6 +66,10 @@ static inline void pair_terms(const orc_params* p, double r2, int pi, int pj, do
   double B = (pi == pj) ? (p->b + p->c) : (p->b - p->c);
   *V = p->a * u * u + B * u;
   *g = (2.0 * p->a * u * u + B * u) / p->Lambda;
+  if (p->r_nuc > 0.0 && !(r2 < p->r_nuc * p->r_nuc)) { /* strict r < r_nuc, plain truncation */
+    *V = 0.0;
+    *g = 0.0;
+  }
   if (pi && pj && r2 > 0.0) {
     double r = sqrt(r2);
     double Ec = p->alpha * exp(-r / p->lambda) / r;

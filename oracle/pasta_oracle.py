@@ -13,7 +13,7 @@ _lib = None
 
 
 class _CParams(C.Structure):
-    _fields_ = [(n, C.c_double) for n in ("a", "b", "c", "Lambda", "alpha", "lambda_", "r_c", "mass")]
+    _fields_ = [(n, C.c_double) for n in ("a", "b", "c", "Lambda", "alpha", "lambda_", "r_c", "mass", "r_nuc")]
 
 
 @dataclass
@@ -28,9 +28,10 @@ class Params:
     lambda_: float = 10.0
     r_c: float = 20.0
     mass: float = 939.0
+    r_nuc: float = 0.0  # > 0: the paper's separate nuclear cut-off (11.5 fm); 0: none (reading D1)
 
     def _c(self):
-        return _CParams(self.a, self.b, self.c, self.Lambda, self.alpha, self.lambda_, self.r_c, self.mass)
+        return _CParams(self.a, self.b, self.c, self.Lambda, self.alpha, self.lambda_, self.r_c, self.mass, self.r_nuc)
 
 
 def build(force=False):

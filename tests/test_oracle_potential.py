@@ -239,3 +239,25 @@ def test_p11_ideal_gas_energy_and_p12_neighbour_count(orc):
     assert expect == pytest.approx(11.27, abs=0.01)  # SURVEY's cfg1 figure
     assert PE / N == pytest.approx(expect, rel=0.06)
     assert d["ordered_pairs"] / N == pytest.approx(n * 4 * math.pi / 3 * 17.0 ** 3, rel=0.01)
+
+
+def test_range_split_of_the_paper(orc):
+    """nuclear terms cut at r_nuc = 11.5 fm, Coulomb not.  Pins of the oracle's r_nuc switch:
+    (i) off by default and equal to the single cut-off reading when r_nuc >= r_c; (ii) beyond r_nuc an np/nn pair
+    feels nothing and a pp pair exactly the Yukawa term alpha exp(-r/lambda)/r with F = V (1/r + 1/lambda);
+    (iii) inside r_nuc nothing changes; (iv) "it will rarely register ... even in 64-bit IEEE arithmetic"
+    (PAPER.md:126): on a config-1 system the split changes no force by more than 1e-19 MeV/fm."""
+    full, split = orc.Params(r_c=17.0), orc.Params(r_c=17.0, r_nuc=11.5)
+    for r in (0.5, 3.0, 11.499):
+        for pi, pj in ((0, 0), (0, 1), (1, 1)):
+            assert orc.pair(split, r, pi, pj) == orc.pair(full, r, pi, pj)
+    for r in (11.5, 12.0, 16.9):
+        assert orc.pair(split, r, 0, 0) == (0.0, 0.0) and orc.pair(split, r, 1, 0) == (0.0, 0.0)
+        V, F = orc.pair(split, r, 1, 1)
+        Vy = 1.44 * math.exp(-r / 10.0) / r
+        assert V == pytest.approx(Vy, rel=1e-14) and F == pytest.approx(Vy * (1.0 / r + 0.1), rel=1e-14)
+    assert orc.pair(orc.Params(r_c=17.0, r_nuc=17.0), 16.0, 0, 1) == orc.pair(full, 16.0, 0, 1)
+    x, v, is_p, L = inputs.config_state(1, seed=4)
+    Ff, ef, pef, _ = orc.forces(x, is_p, L, full)
+    Fs, es, pes, _ = orc.forces(x, is_p, L, split)
+    assert np.abs(Ff - Fs).max() < 1e-19 and abs(pef - pes) < 1e-16
