@@ -63,6 +63,9 @@ typedef struct pasta_params {
                                   underflows FP32 (14.78 fm for Lambda = 1.25) are not streamed: their terms are exactly
                                   0.0f in the kernel's arithmetic, so F and e are unchanged (D23).  0: stream to r_c */
   int32_t reserved1;
+  double r_nuc;                /* > 0: the paper's own range split: the nuclear (Gaussian) terms are zero
+                                  and not computed beyond r_nuc (11.5 fm in the paper) while the Coulomb term still reaches
+                                  r_c.  0 (default): one cut-off r_c for every term (D1).  Must be <= r_c */
 } pasta_params;
 
 /* Device environment: where internal memory and the stream come from. */

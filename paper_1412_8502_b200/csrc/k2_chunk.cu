@@ -77,6 +77,7 @@ struct ChunkArgs {
   int32_t nprim;             // primary entries (some of them empty)
   SpeciesGrid g[2];
   float rcS;     // sigma * r_c
+  float rnS;     // sigma * r_n (cut-off of the nuclear terms)
   float rzeroS;  // scaled distance beyond which exp2(-r'^2) is exactly 0 in FP32 with FTZ (sqrt(126.5))
   const float4* pos4;
   const int32_t* cxyz;
@@ -129,8 +130,8 @@ __device__ __forceinline__ void evaluate(const float4 s, const Targets& t, Accum
   nr2 = __ffma2_rn(neg2(dz), dz, nr2);
   float2 u = make_float2(ex2_approx(nr2.x), ex2_approx(nr2.y));
   if (CUT) {
-    u.x = nr2.x > -c.rc2s ? u.x : 0.f;
-    u.y = nr2.y > -c.rc2s ? u.y : 0.f;
+    u.x = nr2.x > -c.rn2s ? u.x : 0.f;
+    u.y = nr2.y > -c.rn2s ? u.y : 0.f;
   }
   float2 g = __fmul2_rn(u, __ffma2_rn(dup(k.g2a), u, dup(k.gB)));
 #if K2_ESUM
@@ -260,7 +261,7 @@ __device__ __forceinline__ void source_pass(const ChunkArgs& A, const PairConsts
   // np/nn passes without an explicit cut: beyond r'^2 = 126 the pair term is exactly 0 in this arithmetic
   // (ex2.approx.ftz flushes), so sources farther than that from every target need not be streamed at all --
   // the sums are the same to the last bit of every addend (D23).  pp pairs reach out to r_c (Coulomb).
-  const float reach = (COUL || CUT) ? A.rcS : fminf(A.rcS, A.rzeroS);
+  const float reach = COUL ? A.rcS : (CUT ? A.rnS : fminf(A.rcS, A.rzeroS));
   const float rc = reach + slack, rc2 = rc * rc;
   const int my_lo = (int)floorf((b.lo_y - rc) * gs.inv_wS + 0.5f), my_hi = (int)floorf((b.hi_y + rc) * gs.inv_wS + 0.5f);
   const int mz_lo = (int)floorf((b.lo_z - rc) * gs.inv_wS + 0.5f), mz_hi = (int)floorf((b.hi_z + rc) * gs.inv_wS + 0.5f);
@@ -553,6 +554,7 @@ int k2_chunk_forces(Sim* s, bool with_energy, bool stats) {
     A.g[sp].inv_wxS = (float)(1.0 / A.g[sp].wxS_d);
   }
   A.rcS = (float)(sigma * s->prm.r_c);
+  A.rnS = (float)(sigma * (s->prm.r_nuc > 0.0 ? s->prm.r_nuc : s->prm.r_c));
   A.rzeroS = s->prm.skip_exact_zeros ? 11.2472f : 3.0e38f;  // sqrt(126.5): 2^-126.5 is below the FTZ threshold
   A.pos4 = s->pos4.as<float4>();
   A.cxyz = s->cxyz.as<int32_t>();
@@ -562,7 +564,7 @@ int k2_chunk_forces(Sim* s, bool with_energy, bool stats) {
   A.e = s->e.as<double>();
   A.stats = s->counters.as<unsigned long long>() + 10;
   // exp2(-r'^2) is exactly 0 (FTZ) for r'^2 > 126: then np/nn pairs beyond r_c need no explicit cut
-  const bool cut = (double)c.rc2s < 127.0;
+  const bool cut = (double)c.rn2s < 127.0;  // the nuclear cut-off lies inside the FP32 underflow distance
   const int grid = (int)((s->max_chunks + WARPS - 1) / WARPS);
   const dim3 block(WARPS * 32);
   if (stats) PASTA_CUDA_OK(cudaMemsetAsync(A.stats, 0, 3 * sizeof(unsigned long long), s->stream));

@@ -21,6 +21,10 @@ PairConsts make_pair_consts(const pasta_params& p) {
   c.sigma = (float)sigma;
   c.inv_sigma = (float)(1.0 / sigma);
   c.rc2s = (float)(sigma * sigma * p.r_c * p.r_c);
+  {
+    const double rn = p.r_nuc > 0.0 ? p.r_nuc : p.r_c;
+    c.rn2s = (float)(sigma * sigma * rn * rn);
+  }
   c.a = (float)p.a;
   c.g2a = (float)(2.0 * p.a / (p.Lambda * sigma));
   c.B_like = (float)(p.b + p.c);
@@ -50,7 +54,7 @@ __device__ __forceinline__ float fast_rsqrt(float x) {
 template <bool COUL, bool ENERGY>
 __device__ __forceinline__ void pair_accumulate(float dx, float dy, float dz, float r2, float B, float gB,
                                                 const PairConsts& c, float& fx, float& fy, float& fz, float& e) {
-  const float u = fast_ex2(-r2);
+  const float u = r2 < c.rn2s ? fast_ex2(-r2) : 0.f;  // nuclear terms: strict r < r_n
   float g = u * fmaf(c.g2a, u, gB);
   float V = 0.f;
   if (ENERGY) V = u * fmaf(c.a, u, B);
@@ -130,7 +134,7 @@ __global__ void __launch_bounds__(128) k2_v0_kernel(V0Args A, PairConsts c) {
               if (r2 < c.rc2s) {
                 if (COUNT_ONLY) {
                   ++count;
-                  count_nz += (coul || r2 < 126.0f) ? 1 : 0;
+                  count_nz += (coul || (r2 < 126.0f && r2 < c.rn2s)) ? 1 : 0;
                 } else if (coul) {
                   pair_accumulate<true, ENERGY>(ddx, ddy, ddz, r2, B, gB, c, fx, fy, fz, e);
                 } else {
@@ -157,7 +161,7 @@ __global__ void __launch_bounds__(128) k2_v0_kernel(V0Args A, PairConsts c) {
           if (r2 < c.rc2s) {
             if (COUNT_ONLY) {
               ++count;
-              count_nz += (coul || r2 < 126.0f) ? 1 : 0;
+              count_nz += (coul || (r2 < 126.0f && r2 < c.rn2s)) ? 1 : 0;
             } else if (coul) {
               pair_accumulate<true, ENERGY>(ddx, ddy, ddz, r2, B, gB, c, fx, fy, fz, e);
             } else {

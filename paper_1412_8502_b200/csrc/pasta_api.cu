@@ -153,6 +153,7 @@ int pasta_params_default(pasta_params* p) {
   p->auto_grid = 1;
   p->x_subdiv = 0;
   p->skip_exact_zeros = 1;
+  p->r_nuc = 0.0;
   return PASTA_OK;
 }
 
@@ -165,6 +166,10 @@ static int validate_params(const pasta_params* p, double L) {
       p->thermostat_interval < 0 || p->cell_subdiv < 1 || p->cell_subdiv > 64 || p->force_variant < 0) {
     set_error("pasta_params: r_c, Lambda, lambda, mass, scale_per_step must be > 0, thermostat_interval >= 0, "
               "1 <= cell_subdiv <= 64");
+    return PASTA_EINVAL;
+  }
+  if (!(p->r_nuc >= 0.0) || p->r_nuc > p->r_c) {
+    set_error("pasta_params: need 0 <= r_nuc <= r_c");
     return PASTA_EINVAL;
   }
   if (p->r_c > 0.5 * L) {

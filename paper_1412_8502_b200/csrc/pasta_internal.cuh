@@ -81,6 +81,7 @@ struct PairConsts {
   float sigma;       // coordinate pre-scale sqrt(log2(e) / (2 Lambda))
   float inv_sigma;   // 1 / sigma
   float rc2s;        // (sigma r_c)^2
+  float rn2s;        // (sigma r_n)^2, r_n = cut-off of the nuclear terms: r_nuc if set, else r_c
   float a;           // a
   float g2a;         // 2 a / (Lambda sigma)          (force constants carry the 1/sigma of d' -> d)
   float B_like, B_unlike;      // b + c, b - c

@@ -389,3 +389,19 @@ def test_evolved_clustered_state_snapshots(orc, cfg, nsteps, nsample):
             label, n = sim.clusters(c["r_cl"])
             lo, _, _, no = orc.clusters(x, is_p, L, c["r_cl"])
             assert n == no and np.array_equal(_np(label), lo)
+
+
+@pytest.mark.parametrize("variant", [0, 1])
+@pytest.mark.parametrize("N,density,r_c,Y_P", [(2048, 0.05, 17.0, 0.3), (30000, 0.08, 20.0, 0.4)])
+def test_range_split_mode(orc, N, density, r_c, Y_P, variant):
+    """SURVEY 8(f) rank 1, the paper's own range split: nuclear terms cut at r_nuc = 11.5 fm,
+    Coulomb out to r_c.  Same gates as the contract mode, against the oracle run with the same r_nuc."""
+    x, v, is_p, L = inputs.uniform_state(N, Y_P, density, 1.0, seed=21)
+    with _sim_from_arrays(x, v, is_p, L, r_c=r_c, r_nuc=11.5, force_variant=variant) as sim:
+        F, pe = sim.forces()
+        pairs, nonzero = sim.pair_counts()
+    Fo, _, peo, d = orc.forces(x, is_p, L, orc.Params(r_c=r_c, r_nuc=11.5))
+    _check_forces(_np(F), Fo, pe, peo)
+    assert abs(pairs - d["ordered_pairs"]) <= 4 and nonzero < pairs
+    with pytest.raises(pasta.PastaError):
+        pasta.Sim(N, Y_P, density, 1.0, params=pasta.default_params(r_c=r_c, r_nuc=r_c + 1.0), seed=1)
