@@ -11,6 +11,7 @@ from .pasta_oracle import (  # noqa: F401
     cells,
     clusters,
     clusters_cells,
+    clusters_mst,
     composition,
     expand,
     forces,

@@ -341,6 +341,49 @@ void orc_clusters(int64_t N, const double* x, const uint8_t* is_p, double L, dou
 }
 
 /*
+ * O4'. The paper's own "MST" cluster algorithm, brute force:
+ *   (1) protons i, j belong to the same cluster if r_ij <= r_pp (4.5 fm), transitively; a proton with no
+ *       proton in range is its own cluster;
+ *   (2) a neutron is counted as a member of cluster C "if it is within a distance r_np [3 fm] of at least one
+ *       proton j that also belongs to C"; neutrons in no cluster are free (a cluster of their own, A = 1, Z = 0).
+ * Reading D24 (the paper is silent on a neutron within r_np of protons of two clusters): it joins the cluster of
+ * its NEAREST proton (smallest pinned r2; equal r2: the smaller proton index).  Nearest periodic images
+ * throughout, same pinned distance arithmetic as `linked`.  label[i] = smallest PROTON index of
+ * i's cluster (own index for a free neutron); A, Z as in orc_clusters.
+ */
+static inline double pinned_r2(const double* xi, const double* xj, double L, double invL) {
+  double dx = xi[0] - xj[0], dy = xi[1] - xj[1], dz = xi[2] - xj[2];
+  dx = dx - L * rint(dx * invL);
+  dy = dy - L * rint(dy * invL);
+  dz = dz - L * rint(dz * invL);
+  return (dx * dx + dy * dy) + dz * dz;
+}
+void orc_clusters_mst(int64_t N, const double* x, const uint8_t* is_p, double L, double r_pp, double r_np,
+                      int32_t* label, int32_t* A, int32_t* Z, int64_t* n_clusters) {
+  int64_t* parent = (int64_t*)malloc((size_t)N * sizeof(int64_t));
+  const double invL = 1.0 / L, rpp2 = r_pp * r_pp, rnp2 = r_np * r_np;
+  for (int64_t i = 0; i < N; ++i) parent[i] = i;
+  for (int64_t i = 0; i < N; ++i) {
+    if (!is_p[i]) continue;
+    for (int64_t j = i + 1; j < N; ++j)
+      if (is_p[j] && pinned_r2(x + 3 * i, x + 3 * j, L, invL) <= rpp2) uf_union(parent, i, j);
+  }
+  for (int64_t n = 0; n < N; ++n) {
+    if (is_p[n]) continue;
+    int64_t best = -1;
+    double best_r2 = 0.0;
+    for (int64_t j = 0; j < N; ++j) {
+      if (!is_p[j]) continue;
+      const double r2 = pinned_r2(x + 3 * n, x + 3 * j, L, invL);
+      if (r2 <= rnp2 && (best < 0 || r2 < best_r2)) { best = j; best_r2 = r2; }
+    }
+    if (best >= 0) parent[n] = uf_find(parent, best); /* a leaf: nothing is ever hooked under a neutron */
+  }
+  finish_labels(N, parent, is_p, label, A, Z, n_clusters);
+  free(parent);
+}
+
+/*
  * P14 helper: the same components through a cell grid of width >= r_cl (independent pair
  * enumeration; validated against orc_clusters at N <= 4096, then used where N^2 is too slow).
  * Needs floor(L / r_cl) >= 3; returns -1 otherwise.

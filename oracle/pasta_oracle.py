@@ -191,6 +191,22 @@ def clusters(x, is_p, L, r_cl):
     return _clusters(lib.orc_clusters, x, is_p, L, r_cl)
 
 
+def clusters_mst(x, is_p, L, r_pp=4.5, r_np=3.0):
+    """O4': the paper's two-radius MST clusters (reading D24). Returns (label, A, Z, n_clusters)."""
+    x = _f64(x, (-1, 3))
+    is_p = _u8(is_p)
+    N = x.shape[0]
+    label = np.zeros(N, dtype=np.int32)
+    A = np.zeros(N, dtype=np.int32)
+    Z = np.zeros(N, dtype=np.int32)
+    n = C.c_int64()
+    lib = _load()
+    lib.orc_clusters_mst.restype = None
+    lib.orc_clusters_mst(C.c_int64(N), _p(x), _p(is_p), C.c_double(L), C.c_double(r_pp), C.c_double(r_np), _p(label),
+                         _p(A), _p(Z), C.byref(n))
+    return label, A, Z, n.value
+
+
 def clusters_cells(x, is_p, L, r_cl):
     return _clusters(_load().orc_clusters_cells, x, is_p, L, r_cl)
 

@@ -106,3 +106,29 @@ def test_composition_summary(orc):
     c = orc.composition(A, Z, 12)
     assert c["free_n_fraction"] == pytest.approx(2 / 8)
     assert c["n_heavy"] == 2 and c["mean_A"] == 16 and c["sigma_A"] == 4 and c["mean_Z"] == 6 and c["sigma_Z"] == 2
+
+
+def test_mst_clusters_of_the_paper(orc):
+    """PAPER.md:154-158 (reading D24).  Hand-built: two protons 4.4 fm apart form one cluster, a third 4.6 fm further
+    is its own; a neutron 2.9 fm from a proton joins it, one 3.1 fm away is free; neutrons never link neutrons (a
+    chain of neutrons hanging off a proton attaches only its first member); a neutron within r_np of protons of
+    two clusters goes to the nearer one; the periodic image counts.  Invariants on a random state: sum A = N,
+    sum Z = N_p, every cluster with A > 1 has Z >= 1, and with no neutrons the result equals friends-of-friends
+    at r_cl = r_pp."""
+    L = 100.0
+    x = np.array([[10, 10, 10], [14.4, 10, 10], [19.0, 10, 10],      # protons 0, 1 (cluster 0), 2 (own)
+                  [10, 12.9, 10], [10, 13.1 + 2.9, 10],               # neutron 3 joins 0; neutron 4 is 2.9 from 3, 6 from 0: free
+                  [16.6, 10, 10],                                     # neutron 5: 2.2 from proton 1, 2.4 from proton 2 -> cluster 0
+                  [99.0, 10, 10], [1.5, 10, 10]], dtype=float)        # proton 6 and neutron 7 across the face (2.5 fm)
+    is_p = np.array([1, 1, 1, 0, 0, 0, 1, 0], dtype=np.uint8)
+    label, A, Z, n = orc.clusters_mst(x, is_p, L)
+    assert label.tolist() == [0, 0, 2, 0, 4, 0, 6, 6] and n == 4
+    assert (A[0], Z[0]) == (4, 2) and (A[2], Z[2]) == (1, 1) and (A[4], Z[4]) == (1, 0) and (A[6], Z[6]) == (2, 1)
+    x2, _, p2, L2 = inputs.uniform_state(1500, 0.3, 0.01, 1.0, seed=8)
+    label, A, Z, n = orc.clusters_mst(x2, p2, L2)
+    assert A.sum() == 1500 and Z.sum() == p2.sum() and np.all(Z[A > 1] >= 1) and n == np.count_nonzero(A)
+    assert np.all(label[p2 == 1] < p2.sum())                          # clusters are named after protons
+    xp = x2[p2 == 1]
+    lf, Af, Zf, nf = orc.clusters(xp, np.ones(len(xp), np.uint8), L2, 4.5)
+    lm, Am, Zm, nm = orc.clusters_mst(xp, np.ones(len(xp), np.uint8), L2, 4.5, 3.0)
+    assert np.array_equal(lf, lm) and nf == nm
