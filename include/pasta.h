@@ -130,7 +130,16 @@ int pasta_expand(pasta_sim* sim, double scale);
  * EINVAL: r_cl <= 0 or r_cl > L/2.
  */
 int pasta_clusters(pasta_sim* sim, double r_cl, int32_t* label_dev, int64_t* n_clusters_host);
-/* After pasta_clusters: A_dev[r], Z_dev[r] = mass and charge number of the cluster labelled r, 0 elsewhere. */
+/*
+ * The paper's own two-radius "MST" cluster algorithm: protons within r_pp
+ * (4.5 fm) of each other belong to one cluster, transitively; a neutron within r_np (3 fm) of a proton belongs to
+ * that proton's cluster -- to the cluster of its NEAREST proton if several are in range (reading D24); other
+ * neutrons are free (clusters of their own).  Nearest images, the pinned FP64 predicate of pasta_clusters.
+ * label_dev[i] = smallest proton index of i's cluster (i itself for a free neutron).  pasta_cluster_sizes and
+ * pasta_composition apply afterwards.  EINVAL: not 0 < r_np <= r_pp <= L/2.
+ */
+int pasta_clusters_mst(pasta_sim* sim, double r_pp, double r_np, int32_t* label_dev, int64_t* n_clusters_host);
+/* After pasta_clusters / pasta_clusters_mst: A_dev[r], Z_dev[r] = mass and charge number of the cluster labelled r, 0 elsewhere. */
 int pasta_cluster_sizes(pasta_sim* sim, int32_t* A_dev, int32_t* Z_dev);
 /* After pasta_clusters: out6_host = {free-neutron mass fraction #(A=1,Z=0)/N, number of clusters with
  * A >= a_min, mean A, sigma A, mean Z, sigma Z over those clusters}.  Synchronises. */

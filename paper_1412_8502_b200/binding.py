@@ -53,6 +53,7 @@ SIGNATURES = {
     "pasta_step": (C.c_int, [C.c_void_p, C.c_int64, C.c_double]),
     "pasta_expand": (C.c_int, [C.c_void_p, C.c_double]),
     "pasta_clusters": (C.c_int, [C.c_void_p, C.c_double, C.c_void_p, C.POINTER(C.c_int64)]),
+    "pasta_clusters_mst": (C.c_int, [C.c_void_p, C.c_double, C.c_double, C.c_void_p, C.POINTER(C.c_int64)]),
     "pasta_cluster_sizes": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p]),
     "pasta_composition": (C.c_int, [C.c_void_p, C.c_int32, C.POINTER(C.c_double)]),
     "pasta_get_state": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.POINTER(C.c_double),
@@ -203,6 +204,13 @@ class Sim:
         return label, n.value
 
     # -- accessors --------------------------------------------------------------------------------------
+    def clusters_mst(self, r_pp=4.5, r_np=3.0):
+        """The paper's two-radius MST clusters: (label[N] int32 tensor, number of clusters)."""
+        label = self._empty((self.N,), self._torch.int32)
+        n = C.c_int64()
+        _check(self.lib.pasta_clusters_mst(self._h, r_pp, r_np, C.c_void_p(label.data_ptr()), C.byref(n)))
+        return label, n.value
+
     def cluster_sizes(self):
         A = self._empty((self.N,), self._torch.int32)
         Z = self._empty((self.N,), self._torch.int32)

@@ -10,6 +10,16 @@
 
 namespace pasta {
 
+__device__ __forceinline__ double pinned_r2(const double* __restrict__ x, int i, int j, double L, double invL) {
+  double dx = __dsub_rn(x[3 * i + 0], x[3 * j + 0]);
+  double dy = __dsub_rn(x[3 * i + 1], x[3 * j + 1]);
+  double dz = __dsub_rn(x[3 * i + 2], x[3 * j + 2]);
+  dx = __dsub_rn(dx, __dmul_rn(L, rint(__dmul_rn(dx, invL))));
+  dy = __dsub_rn(dy, __dmul_rn(L, rint(__dmul_rn(dy, invL))));
+  dz = __dsub_rn(dz, __dmul_rn(L, rint(__dmul_rn(dz, invL))));
+  return __dadd_rn(__dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy, dy)), __dmul_rn(dz, dz));
+}
+
 __device__ __forceinline__ bool fof_linked(const double* __restrict__ x, int i, int j, double L, double invL,
                                            double rcl2) {
   double dx = __dsub_rn(x[3 * i + 0], x[3 * j + 0]);
@@ -83,9 +93,11 @@ __global__ void k4_scatter_kernel(int64_t N, const int32_t* __restrict__ cell_id
 // One thread per particle i: link with every j < i in the 27 surrounding cells that satisfies the predicate.
 __global__ void k4_link_cells_kernel(int64_t N, const double* __restrict__ x, const int32_t* __restrict__ cell_id,
                                      const int32_t* __restrict__ start, const int32_t* __restrict__ perm, int ncell,
-                                     double L, double invL, double rcl2, int32_t* __restrict__ parent) {
+                                     double L, double invL, double rcl2, int32_t* __restrict__ parent,
+                                     const uint8_t* __restrict__ only) {  // only != NULL: link protons only (MST)
   int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= N) return;
+  if (only && !only[i]) return;
   const int id = cell_id[i];
   const int cx = id % ncell, cy = (id / ncell) % ncell, cz = id / (ncell * ncell);
   for (int dz = -1; dz <= 1; ++dz)
@@ -95,18 +107,61 @@ __global__ void k4_link_cells_kernel(int64_t N, const double* __restrict__ x, co
         const int q = (jz * ncell + jy) * ncell + jx;
         for (int s = start[q]; s < start[q + 1]; ++s) {
           const int j = perm[s];
-          if (j < i && fof_linked(x, j, (int)i, L, invL, rcl2)) uf_union(parent, (int)i, j);
+          if (j < i && (!only || only[j]) && fof_linked(x, j, (int)i, L, invL, rcl2)) uf_union(parent, (int)i, j);
         }
       }
 }
 
+// MST step 2 (reading D24): a neutron joins the cluster of its nearest proton within r_np (smallest
+// pinned r2, then smallest index); it becomes a leaf under that proton -- nothing is ever hooked under a neutron.
+// cell_id == NULL: all protons are scanned (small boxes).
+__global__ void k4_attach_kernel(int64_t N, const double* __restrict__ x, const uint8_t* __restrict__ is_p,
+                                 const int32_t* __restrict__ cell_id, const int32_t* __restrict__ start,
+                                 const int32_t* __restrict__ perm, int ncell, double L, double invL, double rnp2,
+                                 int32_t* __restrict__ parent) {
+  int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= N || is_p[i]) return;
+  int best = -1;
+  double best_r2 = 0.0;
+  if (cell_id) {
+    const int id = cell_id[i];
+    const int cx = id % ncell, cy = (id / ncell) % ncell, cz = id / (ncell * ncell);
+    for (int dz = -1; dz <= 1; ++dz)
+      for (int dy = -1; dy <= 1; ++dy)
+        for (int dx = -1; dx <= 1; ++dx) {
+          const int jx = (cx + dx + ncell) % ncell, jy = (cy + dy + ncell) % ncell, jz = (cz + dz + ncell) % ncell;
+          const int q = (jz * ncell + jy) * ncell + jx;
+          for (int s = start[q]; s < start[q + 1]; ++s) {
+            const int j = perm[s];
+            if (!is_p[j]) continue;
+            const double r2 = pinned_r2(x, (int)i, j, L, invL);
+            if (r2 <= rnp2 && (best < 0 || r2 < best_r2 || (r2 == best_r2 && j < best))) {
+              best = j;
+              best_r2 = r2;
+            }
+          }
+        }
+  } else {
+    for (int j = 0; j < (int)N; ++j) {
+      if (!is_p[j]) continue;
+      const double r2 = pinned_r2(x, (int)i, j, L, invL);
+      if (r2 <= rnp2 && (best < 0 || r2 < best_r2)) {
+        best = j;
+        best_r2 = r2;
+      }
+    }
+  }
+  if (best >= 0) parent[i] = best;
+}
+
 // Small boxes (fewer than 3 cells per side): all pairs j < i.
 __global__ void k4_link_all_kernel(int64_t N, const double* __restrict__ x, double L, double invL, double rcl2,
-                                   int32_t* __restrict__ parent) {
+                                   int32_t* __restrict__ parent, const uint8_t* __restrict__ only) {
   int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= N) return;
+  if (only && !only[i]) return;
   for (int j = 0; j < (int)i; ++j)
-    if (fof_linked(x, j, (int)i, L, invL, rcl2)) uf_union(parent, (int)i, j);
+    if ((!only || only[j]) && fof_linked(x, j, (int)i, L, invL, rcl2)) uf_union(parent, (int)i, j);
 }
 
 __global__ void k4_flatten_kernel(int64_t N, int32_t* __restrict__ parent, const uint8_t* __restrict__ is_p,
@@ -131,8 +186,12 @@ __global__ void k4_store_labels_kernel(int64_t N, int32_t* __restrict__ parent) 
   parent[i] = r;  // r is a root: roots are never rewritten, so concurrent readers still terminate at r
 }
 
-int k4_clusters(Sim* s, double r_cl, int32_t* label_dev, int64_t* n_clusters_host) {
+// r_np > 0: the paper's two-radius MST (protons linked at r_cl = r_pp, neutrons attached at r_np <= r_pp);
+// r_np == 0: friends-of-friends over all nucleons at r_cl.
+int k4_clusters(Sim* s, double r_cl, double r_np, int32_t* label_dev, int64_t* n_clusters_host) {
   const int64_t N = s->N;
+  const bool mst = r_np > 0.0;
+  const uint8_t* only = mst ? s->is_p.as<uint8_t>() : nullptr;
   const int B = 256;
   PASTA_TRY(buffer_reserve(s, &s->cl_parent, sizeof(int32_t) * (size_t)N));
   PASTA_TRY(buffer_reserve(s, &s->cl_A, sizeof(int32_t) * (size_t)N));
@@ -166,11 +225,23 @@ int k4_clusters(Sim* s, double r_cl, int32_t* label_dev, int64_t* n_clusters_hos
                                                            s->cl_perm.as<int32_t>());
     k4_link_cells_kernel<<<grid_for(N, 128), 128, 0, s->stream>>>(N, s->x.as<double>(), s->cl_cell_id.as<int32_t>(),
                                                                   start, s->cl_perm.as<int32_t>(), ncell, L, invL, rcl2,
-                                                                  parent);
+                                                                  parent, only);
     s->launches += 2;
+    if (mst) {
+      k4_attach_kernel<<<grid_for(N, 128), 128, 0, s->stream>>>(N, s->x.as<double>(), s->is_p.as<uint8_t>(),
+                                                                s->cl_cell_id.as<int32_t>(), start,
+                                                                s->cl_perm.as<int32_t>(), ncell, L, invL, r_np * r_np,
+                                                                parent);
+      s->launches += 1;
+    }
   } else {
-    k4_link_all_kernel<<<grid_for(N, 128), 128, 0, s->stream>>>(N, s->x.as<double>(), L, invL, rcl2, parent);
+    k4_link_all_kernel<<<grid_for(N, 128), 128, 0, s->stream>>>(N, s->x.as<double>(), L, invL, rcl2, parent, only);
     s->launches += 1;
+    if (mst) {
+      k4_attach_kernel<<<grid_for(N, 128), 128, 0, s->stream>>>(N, s->x.as<double>(), s->is_p.as<uint8_t>(), nullptr,
+                                                                nullptr, nullptr, 0, L, invL, r_np * r_np, parent);
+      s->launches += 1;
+    }
   }
   k4_flatten_kernel<<<grid_for(N, B), B, 0, s->stream>>>(N, parent, s->is_p.as<uint8_t>(), label_dev,
                                                          s->cl_A.as<int32_t>(), s->cl_Z.as<int32_t>(), counter);

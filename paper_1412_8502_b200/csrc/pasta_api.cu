@@ -335,7 +335,18 @@ int pasta_clusters(pasta_sim* sim, double r_cl, int32_t* label_dev, int64_t* n_c
     return PASTA_EINVAL;
   }
   PASTA_TRY(use_device(s));
-  return k4_clusters(s, r_cl, label_dev, n_clusters_host);
+  return k4_clusters(s, r_cl, 0.0, label_dev, n_clusters_host);
+}
+
+int pasta_clusters_mst(pasta_sim* sim, double r_pp, double r_np, int32_t* label_dev, int64_t* n_clusters_host) {
+  Sim* s = reinterpret_cast<Sim*>(sim);
+  PASTA_TRY(check_sim(s));
+  if (!(r_np > 0.0) || !(r_pp >= r_np) || r_pp > 0.5 * s->L) {
+    set_error("pasta_clusters_mst: need 0 < r_np <= r_pp <= L/2");
+    return PASTA_EINVAL;
+  }
+  PASTA_TRY(use_device(s));
+  return k4_clusters(s, r_pp, r_np, label_dev, n_clusters_host);
 }
 
 int pasta_cluster_sizes(pasta_sim* sim, int32_t* A_dev, int32_t* Z_dev) {

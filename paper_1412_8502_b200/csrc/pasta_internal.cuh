@@ -173,7 +173,7 @@ int k3_kinetic(Sim* s, double* ke_host);
 int k3_sum(Sim* s, const double* in, int64_t n, int slot);  // deterministic sum into scalars[slot]
 int k3_count_protons(Sim* s);                          // s->Np from is_p (synchronises)
 // K4  k4_clusters.cu
-int k4_clusters(Sim* s, double r_cl, int32_t* label_dev, int64_t* n_clusters_host);
+int k4_clusters(Sim* s, double r_cl, double r_np, int32_t* label_dev, int64_t* n_clusters_host);
 int k4_composition(Sim* s, int32_t a_min, double* out6_host);
 
 inline int grid_for(int64_t n, int block) { return (int)((n + block - 1) / block); }

@@ -405,3 +405,20 @@ def test_range_split_mode(orc, N, density, r_c, Y_P, variant):
     assert abs(pairs - d["ordered_pairs"]) <= 4 and nonzero < pairs
     with pytest.raises(pasta.PastaError):
         pasta.Sim(N, Y_P, density, 1.0, params=pasta.default_params(r_c=r_c, r_nuc=r_c + 1.0), seed=1)
+
+
+@pytest.mark.parametrize("N,Y_P,density", [(3000, 0.2, 0.004), (2048, 0.3, 0.05), (40000, 0.3, 0.01)])
+def test_mst_clusters_bit_exact(orc, N, Y_P, density):
+    """the paper's two-radius MST clusters (reading D24) against the oracle on
+    identical positions: labels, cluster count, A and Z bit-exact; also on a clustered stand-in state."""
+    for gen in (inputs.uniform_state, inputs.clustered_state):
+        x, v, is_p, L = gen(N, Y_P, density, 1.0, seed=13)
+        with _sim_from_arrays(x, v, is_p, L, r_c=min(20.0, 0.49 * L)) as sim:
+            label, n = sim.clusters_mst(4.5, 3.0)
+            A, Z = sim.cluster_sizes()
+            comp = sim.composition(12)
+        lo, Ao, Zo, no = orc.clusters_mst(x, is_p, L, 4.5, 3.0)
+        assert n == no and np.array_equal(_np(label), lo)
+        assert np.array_equal(_np(A), Ao) and np.array_equal(_np(Z), Zo)
+        co = orc.composition(Ao, Zo, 12)
+        assert comp["free_n_fraction"] == pytest.approx(co["free_n_fraction"], abs=1e-15) and comp["n_heavy"] == co["n_heavy"]
