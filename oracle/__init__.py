@@ -22,5 +22,6 @@ from .pasta_oracle import (  # noqa: F401
     pair,
     set_num_threads,
     step,
+    step_linear,
     wrap,
 )

@@ -276,6 +276,38 @@ void orc_step(int64_t N, double* x, double* v, const uint8_t* is_p, double* L, c
   }
 }
 
+/*
+ * O2'. The paper's own expansion (Eq. 3a): the side of the box grows linearly in time,
+ * l(t) = l(0) (1 + xi_dot t), and "particle positions and velocities are not incremented with the change in box
+ * volume"; the thermostat is the same.  Reading D25: the box is enlarged right after the drift, before the force
+ * evaluation (PAPER.md:100 says "after the timestep is completed"; like D10, one force evaluation then serves
+ * the closing kick of this step and the opening kick of the next).  n_exp = steps since the expansion began
+ * (in/out); L0 = the side at that moment; t = n_exp * dt with a constant dt.
+ *   (1) v += (dt/2M) F   (2) x = wrap(x + dt v) in the CURRENT box   (3) n_exp += 1; L = L0 (1 + xi_dot dt n_exp)
+ *   (4) F = O1(x, L)     (5) v += (dt/2M) F   (6) thermostat as in O2
+ */
+void orc_step_linear(int64_t N, double* x, double* v, const uint8_t* is_p, double L0, double xi_dot,
+                     int64_t* n_exp, double* L, const orc_params* p, double T, int32_t interval, double dt,
+                     int64_t nsteps, int64_t* step_count, double* F, double* PE) {
+  const double h = dt / (2.0 * p->mass);
+  for (int64_t s = 0; s < nsteps; ++s) {
+    for (int64_t k = 0; k < 3 * N; ++k) v[k] += h * F[k];
+    for (int64_t k = 0; k < 3 * N; ++k) x[k] = wrap_coord(x[k] + dt * v[k], *L);
+    *n_exp += 1;
+    *L = L0 * (1.0 + xi_dot * (dt * (double)(*n_exp)));
+    orc_forces(N, x, is_p, *L, p, 0, NULL, F, NULL, PE, NULL);
+    for (int64_t k = 0; k < 3 * N; ++k) v[k] += h * F[k];
+    *step_count += 1;
+    if (interval > 0 && (*step_count % interval) == 0) {
+      double ke = orc_kinetic(N, v, p->mass);
+      if (ke > 0.0) {
+        double f = sqrt(1.5 * (double)N * T / ke);
+        for (int64_t k = 0; k < 3 * N; ++k) v[k] *= f;
+      }
+    }
+  }
+}
+
 /* One-shot uniform scaling (pasta_expand): L *= s, x *= s, v untouched (reading D9). */
 void orc_expand(int64_t N, double* x, double* L, double s) {
   *L = (*L) * s;

@@ -163,6 +163,24 @@ def step(x, v, is_p, L, params, T, interval, scale_per_step, dt, nsteps, step_co
     return x, v, Lc.value, cnt.value, F, PE.value
 
 
+def step_linear(x, v, is_p, L0, xi_dot, params, T, interval, dt, nsteps, n_exp=0, step_count=0, F=None):
+    """O2': the paper's linear box-only expansion (Eq. 3a; reading D25).
+    Returns (x, v, L, n_exp, step_count, F, PE) after nsteps; inputs are not modified."""
+    x = _f64(x, (-1, 3)).copy()
+    v = _f64(v, (-1, 3)).copy()
+    is_p = _u8(is_p)
+    N = x.shape[0]
+    L = L0 * (1.0 + xi_dot * (dt * float(n_exp)))
+    if F is None:
+        F = forces(x, is_p, L, params)[0]
+    F = _f64(F, (-1, 3)).copy()
+    Lc, ne, cnt, PE = C.c_double(L), C.c_int64(n_exp), C.c_int64(step_count), C.c_double(0.0)
+    _load().orc_step_linear(C.c_int64(N), _p(x), _p(v), _p(is_p), C.c_double(L0), C.c_double(xi_dot), C.byref(ne),
+                            C.byref(Lc), C.byref(params._c()), C.c_double(T), C.c_int32(interval), C.c_double(dt),
+                            C.c_int64(nsteps), C.byref(cnt), _p(F), C.byref(PE))
+    return x, v, Lc.value, ne.value, cnt.value, F, PE.value
+
+
 def expand(x, L, s):
     x = _f64(x, (-1, 3)).copy()
     Lc = C.c_double(L)

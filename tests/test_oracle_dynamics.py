@@ -161,3 +161,35 @@ def test_maxwell_boltzmann_inputs():
     assert v.var() == pytest.approx(1.0 / 939.0, rel=4 * math.sqrt(2.0 / v.size))
     assert (x >= 0).all() and (x < L).all()
     assert inputs.n_protons(2048, 0.30) == 614 and inputs.n_protons(409600, 0.30) == 122880
+
+
+def test_linear_box_only_expansion_of_the_paper(orc):
+    """PAPER.md:100-108, Eq. 3a (reading D25).  Pins: (i) l(t) = l(0)(1 + xi_dot t) exactly as written, after any
+    number of steps and across calls; (ii) positions are NOT scaled: with the potential switched off a particle
+    that crosses no face moves as x0 + v t to rounding while the box grows by 50 %; (iii) a particle that does
+    cross re-enters at x - L of the box it left, with its velocity unchanged; (iv) xi_dot = 0 is
+    plain velocity Verlet (identical to orc.step with s = 1)."""
+    free = orc.Params(a=0.0, b=0.0, c=0.0, alpha=0.0, r_c=5.0)
+    L0, xi, dt = 40.0, 5e-3, 2.0
+    x = np.array([[10.0, 20.0, 30.0], [39.5, 5.0, 5.0]])
+    v = np.array([[0.01, -0.02, 0.005], [0.1, 0.0, 0.0]])
+    is_p = np.array([1, 0], dtype=np.uint8)
+    xo, vo, L, ne, cnt, F, pe = orc.step_linear(x, v, is_p, L0, xi, free, 1.0, 0, dt, 50)
+    assert L == L0 * (1.0 + xi * (dt * 50.0)) and ne == 50 and cnt == 50
+    assert np.allclose(xo[0], x[0] + v[0] * 100.0, rtol=0, atol=1e-12) and np.array_equal(vo, v)
+    # particle 1 leaves the box of side L0 (1 + xi dt 2) = 40.8 during step 3 (x = 40.1 after it is drifted in a
+    # box that has grown twice) ... track it by hand
+    xs, Ls = 39.5, L0
+    for n in range(1, 51):
+        xs = xs + 0.1 * dt
+        if xs >= Ls:
+            xs -= Ls
+        Ls = L0 * (1.0 + xi * (dt * n))
+    assert xo[1, 0] == pytest.approx(xs, abs=1e-12)
+    x2, v2, L2, ne2, cnt2, _, _ = orc.step_linear(xo, vo, is_p, L0, xi, free, 1.0, 0, dt, 25, n_exp=ne, step_count=cnt)
+    assert L2 == L0 * (1.0 + xi * (dt * 75.0)) and ne2 == 75
+    xr, vr, isr, Lr = inputs.uniform_state(64, 0.3, 0.02, 1.0, seed=3)
+    prm = orc.Params(r_c=5.0)
+    a = orc.step_linear(xr, vr, isr, Lr, 0.0, prm, 1.0, 10, 2.0, 12)
+    b = orc.step(xr, vr, isr, Lr, prm, 1.0, 10, 1.0, 2.0, 12)
+    assert np.array_equal(a[0], b[0]) and np.array_equal(a[1], b[1]) and a[2] == b[2]
