@@ -66,6 +66,10 @@ typedef struct pasta_params {
   double r_nuc;                /* > 0: the paper's own range split: the nuclear (Gaussian) terms are zero
                                   and not computed beyond r_nuc (11.5 fm in the paper) while the Coulomb term still reaches
                                   r_c.  0 (default): one cut-off r_c for every term (D1).  Must be <= r_c */
+  double xi_dot;               /* > 0: the paper's own expansion (Eq. 3a; D25): after the drift of every step
+                                  the box side becomes L0 (1 + xi_dot dt n), n = steps since create / set_state / expand and
+                                  L0 the side at that moment; positions and velocities are NOT scaled.  Needs
+                                  scale_per_step == 1 and a constant dt.  0 (default): off */
 } pasta_params;
 
 /* Device environment: where internal memory and the stream come from. */

@@ -110,13 +110,14 @@ static int red_blocks(int64_t n) {
   return (int)(b < 1 ? 1 : (b > 1184 ? 1184 : b));  // 148 SMs x 8 resident blocks
 }
 
-// The caller has set s->L to the box of the NEW positions.
-int k3_kick_drift_count(Sim* s, double dt, double scale) {
+// The caller has set s->L to the box the forces will be evaluated in; L_wrap = the box the drifted positions are
+// wrapped into (the same, except under the linear box-only expansion, where it is the box before it grew).
+int k3_kick_drift_count(Sim* s, double dt, double scale, double L_wrap) {
   GridPair g;
   PASTA_TRY(k1_setup(s, false, &g));
   k3_kick_drift_count_kernel<<<grid_for(s->N, 128), 128, 0, s->stream>>>(
       s->N, s->x.as<double>(), s->v.as<double>(), s->F.as<double>(), s->is_p.as<uint8_t>(), dt / (2.0 * s->prm.mass),
-      dt, scale, s->L, 1.0 / s->L, g, s->cell_id.as<int32_t>(), s->bin_count.as<int32_t>());
+      dt, scale, L_wrap, 1.0 / L_wrap, g, s->cell_id.as<int32_t>(), s->bin_count.as<int32_t>());
   s->launches += 1;
   s->hist_valid = true;
   s->hist_uniform = s->prm.force_variant == 1;

@@ -154,6 +154,7 @@ int pasta_params_default(pasta_params* p) {
   p->x_subdiv = 0;
   p->skip_exact_zeros = 1;
   p->r_nuc = 0.0;
+  p->xi_dot = 0.0;
   return PASTA_OK;
 }
 
@@ -170,6 +171,10 @@ static int validate_params(const pasta_params* p, double L) {
   }
   if (!(p->r_nuc >= 0.0) || p->r_nuc > p->r_c) {
     set_error("pasta_params: need 0 <= r_nuc <= r_c");
+    return PASTA_EINVAL;
+  }
+  if (!(p->xi_dot >= 0.0) || (p->xi_dot > 0.0 && p->scale_per_step != 1.0)) {
+    set_error("pasta_params: need xi_dot >= 0, and scale_per_step == 1 when xi_dot > 0");
     return PASTA_EINVAL;
   }
   if (p->r_c > 0.5 * L) {
@@ -213,6 +218,8 @@ int pasta_create(pasta_sim** out, int64_t N, double Y_P, double density, double 
   s->Np = (int64_t)floor(Y_P * (double)N + 0.5);
   s->T = T;
   s->L = L;
+  s->lin_L0 = L;
+  s->lin_n = 0;
   int rc = PASTA_OK;
   do {
     int ndev = 0;
@@ -288,7 +295,9 @@ int pasta_step(pasta_sim* sim, int64_t n, double dt) {
   const bool energy = s->prm.energy_every_step != 0;
   if (n > 0 && !s->forces_valid) PASTA_TRY(evaluate_forces(s, energy));
   for (int64_t k = 0; k < n; ++k) {
-    const double L_new = sc * s->L;
+    const double L_old = s->L;
+    const bool linear = s->prm.xi_dot > 0.0;
+    const double L_new = linear ? s->lin_L0 * (1.0 + s->prm.xi_dot * (dt * (double)(s->lin_n + 1))) : sc * s->L;
     if (s->prm.r_c > 0.5 * L_new) {
       set_error("pasta_step: box side %g would fall below 2 r_c", L_new);
       return PASTA_EINVAL;
@@ -296,7 +305,8 @@ int pasta_step(pasta_sim* sim, int64_t n, double dt) {
     s->L = L_new;
     {
       Timer t(s, 2);
-      PASTA_TRY(k3_kick_drift_count(s, dt, sc));
+      PASTA_TRY(k3_kick_drift_count(s, dt, sc, linear ? L_old : L_new));
+      s->lin_n += 1;
     }
     s->clusters_valid = false;
     PASTA_TRY(evaluate_forces(s, energy));
@@ -321,6 +331,8 @@ int pasta_expand(pasta_sim* sim, double scale) {
   const double L_new = s->L * scale;
   PASTA_TRY(k3_wrap_scale(s, scale, L_new));
   s->L = L_new;
+  s->lin_L0 = L_new;
+  s->lin_n = 0;
   s->forces_valid = false;
   s->energies_valid = false;
   s->clusters_valid = false;
@@ -394,6 +406,8 @@ int pasta_get_state(pasta_sim* sim, double* x_dev, double* v_dev, uint8_t* is_pr
 
 static int after_set_state(Sim* s, bool have_is_p, bool have_F, double L) {
   s->L = L;
+  s->lin_L0 = L;
+  s->lin_n = 0;
   PASTA_TRY(k3_wrap_scale(s, 1.0, L));
   if (have_is_p) {
     PASTA_TRY(k3_count_protons(s));  // the sorted layout needs the new proton count on the host

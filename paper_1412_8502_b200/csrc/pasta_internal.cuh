@@ -104,6 +104,8 @@ struct Sim {
   double T = 0.0;
   double L = 0.0;
   int64_t step_count = 0;
+  double lin_L0 = 0.0;   // linear expansion (xi_dot > 0): side and step count at its start
+  int64_t lin_n = 0;
   bool forces_valid = false;
   bool energies_valid = false;
   bool clusters_valid = false;
@@ -166,7 +168,8 @@ int k2_reference_forces(Sim* s, bool with_energy);     // variant 1: thread per 
 int k2_chunk_forces(Sim* s, bool with_energy, bool stats);  // variant 2: chunk kernel (k2_chunk.cu)
 // K3  k3_integrate.cu
 int k3_init_state(Sim* s, uint64_t seed);
-int k3_kick_drift_count(Sim* s, double dt, double scale);  // kick, drift, scale, wrap for box s->L + cell histogram
+int k3_kick_drift_count(Sim* s, double dt, double scale, double L_wrap);  // kick, drift, scale, wrap into [0, L_wrap);
+                                                                         // cell histogram on the grids of box s->L
 int k3_kick_ke(Sim* s, double dt, bool rescale);       // second half kick + KE (+ rescale)
 int k3_wrap_scale(Sim* s, double scale, double L_new); // x = wrap(scale x)
 int k3_kinetic(Sim* s, double* ke_host);

@@ -422,3 +422,25 @@ def test_mst_clusters_bit_exact(orc, N, Y_P, density):
         assert np.array_equal(_np(A), Ao) and np.array_equal(_np(Z), Zo)
         co = orc.composition(Ao, Zo, 12)
         assert comp["free_n_fraction"] == pytest.approx(co["free_n_fraction"], abs=1e-15) and comp["n_heavy"] == co["n_heavy"]
+
+
+def test_linear_box_only_expansion_mode(orc):
+    """the paper's expansion law (Eq. 3a; reading D25) -- box side
+    L0 (1 + xi_dot t), positions and velocities not scaled -- against the oracle's step_linear: 20 steps from a
+    config-1 state with a (deliberately fast) xi_dot, thermostat every 10 steps, across two pasta_step calls."""
+    c = inputs.CONFIGS[1]
+    x, v, is_p, L = inputs.config_state(1, seed=5)
+    xi = 2.0e-4
+    with _sim_from_arrays(x, v, is_p, L, T=c["T"], r_c=c["r_c"], xi_dot=xi, thermostat_interval=10) as sim:
+        sim.step(12, c["dt"])
+        sim.step(8, c["dt"])
+        xg, vg, _, Lg, step = sim.get_state()
+        xg, vg = _np(xg), _np(vg)
+    xo, vo, Lo, ne, cnt, _, _ = orc.step_linear(x, v, is_p, L, xi, orc.Params(r_c=c["r_c"]), c["T"], 10, c["dt"], 20)
+    assert Lg == Lo == L * (1.0 + xi * (c["dt"] * 20.0)) and step == cnt == 20
+    d = xg - xo
+    d -= Lo * np.round(d / Lo)
+    assert np.linalg.norm(d, axis=1).max() <= TRAJ_TOL
+    assert np.abs(vg - vo).max() <= 1e-5  # 1e-4 fm over 40 fm/c of a chaotic trajectory
+    with pytest.raises(pasta.PastaError):
+        pasta.Sim(2048, 0.3, 0.05, 1.0, params=pasta.default_params(r_c=17.0, xi_dot=1e-5, scale_per_step=1.0001), seed=1)
