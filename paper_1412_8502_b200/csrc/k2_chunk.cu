@@ -1,9 +1,10 @@
 // K2, production variant -- "chunk" pair-force kernel for sm_100a.
 //
 // Work decomposition:
-//   * a CHUNK is T = 8 consecutive same-species particles of the cell-sorted order.  The force grids are
-//     sliced into thin cells along x, so a row of cells (fixed cy, cz) is sorted in x and a chunk is a
-//     short stretch of one row: spatially compact.  One warp owns one chunk.
+//   * a CHUNK is up to T = 8 same-species particles that lie close together, listed in the chunk table that K1
+//     builds (k1_cells.cu): in a dense system a short stretch of one row of cells (the force grids are sliced
+//     into thin cells along x, so a row -- fixed cy, cz -- is sorted in x), in a sparse one the particles of a
+//     small block of cells.  One warp owns one chunk.
 //   * SOURCES: for each source species the warp lists the rows of that species' grid that can hold a
 //     particle within r_c of the chunk's bounding box, and for every row the tight range of thin cells
 //     [lo_x - xr, hi_x + xr]; a range is contiguous in the sorted arrays, i.e. one segment of slots (two
@@ -14,7 +15,7 @@
 //     list, plain 16-byte load one tile ahead), shifts it into the chunk's frame and stores it in a
 //     double-buffered shared-memory tile.
 //   * CONSUMER side: lane = (target pair p, phase h), p = lane / 8, h = lane % 8.  A lane keeps ONE packed
-//     pair of targets and their accumulators in registers (about 50 registers in all, so 8 warps per SM
+//     pair of targets and their accumulators in registers (96 registers per thread in all, 5 warps per SM
 //     sub-partition are resident) and evaluates sources h, h + 8, h + 16, h + 24 of the tile against them
 //     with packed FP32 arithmetic (FFMA2/FADD2/FMUL2: two pairs per issued instruction).
 //   * There is NO per-candidate test and no divergence: a source that is out of range of a target
@@ -34,9 +35,6 @@ namespace {
 #endif
 #ifndef K2_MINB
 #define K2_MINB 5
-#endif
-#ifndef K2_ESUM
-#define K2_ESUM 0
 #endif
 #ifndef K2_WARPS
 #define K2_WARPS 4
@@ -107,11 +105,8 @@ struct WarpShared {
 struct Targets {
   float2 ntx, nty, ntz;
 };
-// The nuclear energy of a pass is a S2 + B S1 with S1 = sum u, S2 = sum u^2 (B is constant over a pass), which
-// costs two 2-operand packed instructions per step instead of a polynomial and a 3-operand accumulate;
-// `e` holds the energy of the finished passes plus the Coulomb terms.
 struct Accum {
-  float2 fx, fy, fz, e, s1, s2;
+  float2 fx, fy, fz, e;
 };
 struct PassConsts {
   float g2a, gB, a, B;
@@ -134,14 +129,7 @@ __device__ __forceinline__ void evaluate(const float4 s, const Targets& t, Accum
     u.y = nr2.y > -c.rn2s ? u.y : 0.f;
   }
   float2 g = __fmul2_rn(u, __ffma2_rn(dup(k.g2a), u, dup(k.gB)));
-#if K2_ESUM
-  if (ENERGY) {
-    acc.s1 = __fadd2_rn(acc.s1, u);
-    acc.s2 = __ffma2_rn(u, u, acc.s2);
-  }
-#else
   if (ENERGY) acc.e = __ffma2_rn(u, __ffma2_rn(dup(k.a), u, dup(k.B)), acc.e);
-#endif
   if (COUL) {
     // screened Coulomb, cut at r_c, skipped at r = 0 (the self pair and coincident protons, D2):
     // 1/r' := 0 for excluded pairs, which zeroes every Coulomb factor without creating inf * 0
@@ -437,10 +425,6 @@ __device__ __forceinline__ void chunk_passes(const ChunkArgs& A, const PairConst
       source_pass<true, CUT, ENERGY, STATS>(A, c, sh, lane, gs, rx, ry, rz, b, t, acc, k, st);
     else
       source_pass<false, CUT, ENERGY, STATS>(A, c, sh, lane, gs, rx, ry, rz, b, t, acc, k, st);
-    if (ENERGY && K2_ESUM) {  // nuclear energy of this pass: a S2 + B S1
-      acc.e = __ffma2_rn(dup(k.a), acc.s2, __ffma2_rn(dup(k.B), acc.s1, acc.e));
-      acc.s1 = acc.s2 = make_float2(0.f, 0.f);
-    }
   }
 }
 
@@ -472,7 +456,7 @@ __global__ void __launch_bounds__(WARPS * 32, K2_MINB) k2_chunk_kernel(const Chu
   const int tc = __ldg(A.cxyz + tslot);
 
   Accum acc;
-  acc.fx = acc.fy = acc.fz = acc.e = acc.s1 = acc.s2 = make_float2(0.f, 0.f);
+  acc.fx = acc.fy = acc.fz = acc.e = make_float2(0.f, 0.f);
   unsigned long long st[3] = {0, 0, 0};
 
   chunk_passes<CUT, ENERGY, STATS>(A, c, sh, lane, pr, gt, st_sp, chunk_p, tp, tc, active, acc, st);
