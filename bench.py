@@ -233,7 +233,8 @@ def run_ours(args, rank, world, local_rank):
     launches = sim.launch_count() - n0
     tm = sim.get_timing()
     sim.set_timing(False)
-    dev_s = sum(a.elapsed_time(b) for a, b in ev) * 1e-3
+    per_step_ms = sorted(a.elapsed_time(b) for a, b in ev)
+    dev_s = sum(per_step_ms) * 1e-3
     pairs, pairs_nz = sim.pair_counts()  # ordered in-range pairs; those with a term that is not exactly 0 in FP32
     ke, pe = sim.energy()
 
@@ -270,6 +271,7 @@ def run_ours(args, rank, world, local_rank):
         line = {
             "metric": "md_steps_per_s", "value": steps_per_s, "unit": "steps/s", "n_gpus": world,
             "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": 1e3 * dev_s / args.steps,
+            "ms_per_step_stats": {"median": statistics.median(per_step_ms), "min": per_step_ms[0], "max": per_step_ms[-1]},
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
             "config": workload_config(args.config, world),
             "pair_interactions_per_s": {"unordered": 0.5 * pairs * steps_per_s, "ordered": pairs * steps_per_s,
