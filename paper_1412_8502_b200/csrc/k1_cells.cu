@@ -222,7 +222,7 @@ __global__ void k1_gather_kernel(int64_t N, const double* __restrict__ x, const 
 //   SPARSE (blocks): 8 consecutive particles of a row would be far apart, so the particles of a block of B x B x B
 //          cells (B w <= 20 fm) are grouped instead, 8 at a time; one thread per block, entries in the overflow
 //          region, reserved once per warp.
-constexpr int CHUNK_T = 8;
+constexpr int CHUNK_T = PASTA_CHUNK_T;
 struct ChunkGeom {
   int xmax[2];   // DENSE: extent limit of a chunk in thin cells
   int block[2];  // 0 = DENSE, else B of the SPARSE builder
@@ -230,11 +230,15 @@ struct ChunkGeom {
 };
 
 __device__ __forceinline__ void write_entry(int32_t* __restrict__ tab, int64_t e, int first, int n) {
-  int4 a, b;
-  a.x = n > 0 ? first : -1; a.y = n > 1 ? first + 1 : -1; a.z = n > 2 ? first + 2 : -1; a.w = n > 3 ? first + 3 : -1;
-  b.x = n > 4 ? first + 4 : -1; b.y = n > 5 ? first + 5 : -1; b.z = n > 6 ? first + 6 : -1; b.w = n > 7 ? first + 7 : -1;
-  reinterpret_cast<int4*>(tab + e * CHUNK_T)[0] = a;
-  reinterpret_cast<int4*>(tab + e * CHUNK_T)[1] = b;
+#pragma unroll
+  for (int k = 0; k < CHUNK_T; k += 4) {
+    int4 a;
+    a.x = n > k ? first + k : -1;
+    a.y = n > k + 1 ? first + k + 1 : -1;
+    a.z = n > k + 2 ? first + k + 2 : -1;
+    a.w = n > k + 3 ? first + k + 3 : -1;
+    reinterpret_cast<int4*>(tab + e * CHUNK_T)[k / 4] = a;
+  }
 }
 
 __global__ void k1_chunk_rows_kernel(int32_t N, int32_t Np, const int32_t* __restrict__ cxyz,
@@ -328,7 +332,7 @@ __global__ void k1_chunk_blocks_kernel(int sp, const int32_t* __restrict__ bin_s
 // Cells per side of a species' grid: the O3 formula with the k that puts about CHUNK particles in a cell.
 static int auto_subdiv(double L, double r_c, int64_t n_species, int k_default) {
   if (n_species <= 0) return k_default;
-  const double w_star = L * cbrt(8.0 / (double)n_species);
+  const double w_star = L * cbrt((double)PASTA_CHUNK_T / (double)n_species);
   int k = (int)floor(r_c / w_star + 0.5);
   // never wider than 8 fm: sorted coordinates are FP32 offsets from the cell centre, and their quantum
   // (2^-24 of the half width) times the steepest pair-force gradient (~80 MeV/fm^2 inside a cluster) has to

@@ -30,9 +30,7 @@ namespace pasta {
 
 namespace {
 
-#ifndef K2_T
-#define K2_T 8
-#endif
+#define K2_T PASTA_CHUNK_T
 #ifndef K2_MINB
 #define K2_MINB 5
 #endif

@@ -7,6 +7,11 @@
 
 #include "pasta.h"
 
+// targets per chunk of the pair kernel (k1_cells.cu builds the table, k2_chunk.cu consumes it)
+#ifndef PASTA_CHUNK_T
+#define PASTA_CHUNK_T 8
+#endif
+
 namespace pasta {
 
 // ---- error plumbing ------------------------------------------------------------------------------
