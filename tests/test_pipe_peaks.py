@@ -1,0 +1,30 @@
+"""The denominators of the K2 roofline, measured (profiles/r1_pipe_microbench.md): the FP32 pipe
+issues one scalar warp instruction per clock per SM sub-partition (128 lanes/clk/SM), MUFU.EX2 one per 8 clocks
+(16/clk/SM), a packed FFMA2/FADD2/FMUL2 occupies the pipe for 2 clocks (3 with three distinct register-pair
+operands), and the pair-evaluation step of k2_chunk.cu costs 31-34 clocks from registers."""
+import os
+import subprocess
+
+import pytest
+
+pytestmark = pytest.mark.gpu
+HERE = os.path.dirname(os.path.abspath(__file__))
+
+
+def test_pipe_throughputs(tmp_path):
+    exe = str(tmp_path / "pipes")
+    subprocess.check_call([os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc"), "-gencode", "arch=compute_100a,code=sm_100a",
+                           "-O3", "-o", exe, os.path.join(HERE, "ubench", "pipes.cu")], stderr=subprocess.DEVNULL)
+    out = subprocess.run([exe], capture_output=True, text=True, timeout=120, check=True).stdout
+    r = {}
+    for line in out.splitlines():
+        f = line.split()
+        if len(f) == 3 and f[1].startswith("W="):
+            r[(f[0], int(f[1][2:]))] = float(f[2])
+    print(out)
+    assert r[("mufu_ex2", 8)] == pytest.approx(8.0, rel=0.03)            # 4 lanes/clk/SMSP = 16/clk/SM
+    assert 1.0 <= r[("ffma", 8)] <= 1.3                                   # 32 lanes/clk/SMSP = 128/clk/SM
+    assert r[("ffma2_2op", 8)] == pytest.approx(2.0, rel=0.05)            # packed: same lane throughput
+    assert r[("fadd2_bcast", 8)] == pytest.approx(2.0, rel=0.05) and r[("fmul2", 8)] == pytest.approx(2.0, rel=0.05)
+    assert r[("ffma2_3op", 8)] == pytest.approx(3.0, rel=0.05)            # register-file read bandwidth
+    assert 29.0 <= r[("eval_step", 8)] <= 36.0                            # 13 packed + 2 MUFU: pipe-bound
