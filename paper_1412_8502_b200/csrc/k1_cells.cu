@@ -461,6 +461,7 @@ int k1_build(Sim* s, bool uniform_grid) {
       }
     }
     cg.nprim = any_rows ? (int)((N + CHUNK_T - 1) / CHUNK_T) : 0;
+    s->chunks_sparse = (cg.block[0] != 0 && s->Np > 0) || (cg.block[1] != 0 && N - s->Np > 0);
     s->chunk_nprim = cg.nprim;
     s->max_chunks = cg.nprim + overflow;
     PASTA_TRY(buffer_reserve(s, &s->chunk_tab, sizeof(int32_t) * CHUNK_T * (size_t)(s->max_chunks + 8)));

@@ -34,6 +34,9 @@ namespace {
 #ifndef K2_MINB
 #define K2_MINB 5
 #endif
+#ifndef K2_MINB_SPARSE
+#define K2_MINB_SPARSE 8
+#endif
 #ifndef K2_WARPS
 #define K2_WARPS 4
 #endif
@@ -426,8 +429,11 @@ __device__ __forceinline__ void chunk_passes(const ChunkArgs& A, const PairConst
   }
 }
 
-template <bool CUT, bool ENERGY, bool STATS>
-__global__ void __launch_bounds__(WARPS * 32, K2_MINB) k2_chunk_kernel(const ChunkArgs A, const PairConsts c) {
+// MINB = resident blocks per SM the registers are budgeted for: K2_MINB (96 registers) where chunks stream hundreds
+// of tiles and the arithmetic loop sets the pace; K2_MINB_SPARSE (64 registers, 60 % more warps) where a species is
+// sparse, chunks stream a handful of tiles and the latency of the listing does.
+template <bool CUT, bool ENERGY, bool STATS, int MINB>
+__global__ void __launch_bounds__(WARPS * 32, MINB) k2_chunk_kernel(const ChunkArgs A, const PairConsts c) {
   __shared__ WarpShared shared[WARPS];
   const int lane = threadIdx.x & 31;
   // the warp index is produced by REDUX so that the compiler can prove it warp-uniform and keep it (and
@@ -550,7 +556,11 @@ int k2_chunk_forces(Sim* s, bool with_energy, bool stats) {
   const int grid = (int)((s->max_chunks + WARPS - 1) / WARPS);
   const dim3 block(WARPS * 32);
   if (stats) PASTA_CUDA_OK(cudaMemsetAsync(A.stats, 0, 3 * sizeof(unsigned long long), s->stream));
-#define PASTA_K2_LAUNCH(CUT_, EN_, ST_) k2_chunk_kernel<CUT_, EN_, ST_><<<grid, block, 0, s->stream>>>(A, c)
+#define PASTA_K2_LAUNCH(CUT_, EN_, ST_)                                                                       \
+  do {                                                                                                        \
+    if (s->chunks_sparse) k2_chunk_kernel<CUT_, EN_, ST_, K2_MINB_SPARSE><<<grid, block, 0, s->stream>>>(A, c); \
+    else k2_chunk_kernel<CUT_, EN_, ST_, K2_MINB><<<grid, block, 0, s->stream>>>(A, c);                       \
+  } while (0)
   if (stats) {
     if (cut) PASTA_K2_LAUNCH(true, true, true);
     else PASTA_K2_LAUNCH(false, true, true);

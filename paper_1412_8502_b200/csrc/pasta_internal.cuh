@@ -149,6 +149,7 @@ struct Sim {
   Buffer chunk_tab;
   int64_t max_chunks = 0;   // launch bound of the pair kernel: chunk_nprim primary entries + overflow capacity
   int64_t chunk_nprim = 0;
+  bool chunks_sparse = false;  // some species' chunks come from the SPARSE (cell block) builder
 
   // timing: pairs of events (start, stop) tagged with the kernel group they bracket
   bool timing = false;

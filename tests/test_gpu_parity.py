@@ -34,14 +34,39 @@ def _oparams(orc, p):
                       mass=p.mass)
 
 
-def _check_forces(F_gpu, F_orc, pe_gpu=None, pe_orc=None):
-    """D17: (i) ||dF||_2/||F||_2 over the 3N vector; (ii) per particle |dF_i| <= tol max(|F_i|, F_rms)."""
-    dF = F_gpu - F_orc
-    rel = np.linalg.norm(dF) / np.linalg.norm(F_orc)
-    assert rel <= FORCE_TOL, "force relative L2 error %.3e" % rel
+def _alts(orc, x, is_p, L, op, targets=None):
+    """Oracle forces for r_c (1 -+ 3e-7) (see _check_forces), computed only when the plain comparison fails."""
+    def run():
+        out = []
+        for f in (1.0 - 3e-7, 1.0 + 3e-7):
+            pa = orc.Params(**{k: getattr(op, k) for k in ("a", "b", "c", "Lambda", "alpha", "lambda_", "r_c", "mass", "r_nuc")})
+            pa.r_c = op.r_c * f
+            out.append(orc.forces(x, is_p, L, pa, targets=targets)[0])
+        return out
+    return run
+
+
+def _check_forces(F_gpu, F_orc, pe_gpu=None, pe_orc=None, alternates=None):
+    """D17: (i) ||dF||_2/||F||_2 over the 3N vector; (ii) per particle |dF_i| <= tol max(|F_i|, F_rms).
+    `alternates` (from _alts): oracle forces for r_c (1 +- 3e-7).  Reading D22: the GPU decides r < r_c on FP32
+    cell-relative coordinates, so a proton pair within ~1e-6 fm of r_c may fall on the other side of the plain
+    truncation (D1), a jump of F_c(r_c) = 1.5e-3 MeV/fm in two forces; such a particle must then agree with the
+    oracle run at a cut-off moved by less than the FP32 resolution of r."""
     fi = np.linalg.norm(F_orc, axis=1)
     frms = math.sqrt((fi ** 2).mean())
-    worst = (np.linalg.norm(dF, axis=1) / np.maximum(fi, frms)).max()
+
+    def gates(dF):
+        return np.linalg.norm(dF) / np.linalg.norm(F_orc), (np.linalg.norm(dF, axis=1) / np.maximum(fi, frms)).max()
+
+    dF = F_gpu - F_orc
+    rel, worst = gates(dF)
+    if (rel > FORCE_TOL or worst > FORCE_TOL) and alternates is not None:
+        for Fa in alternates():
+            da = F_gpu - Fa
+            better = np.linalg.norm(da, axis=1) < np.linalg.norm(dF, axis=1)
+            dF = np.where(better[:, None], da, dF)
+        rel, worst = gates(dF)
+    assert rel <= FORCE_TOL, "force relative L2 error %.3e" % rel
     assert worst <= FORCE_TOL, "worst per-particle force error %.3e" % worst
     if pe_orc is not None:
         assert abs(pe_gpu - pe_orc) <= PE_TOL * abs(pe_orc), "PE %r vs %r" % (pe_gpu, pe_orc)
@@ -70,7 +95,7 @@ def test_config1_forces_energy_cells(orc, k, variant):
         assert (x >= 0).all() and (x < L).all()
         F, pe = sim.forces()
         Fo, eo, peo, d = orc.forces(x, is_p, L, _oparams(orc, p))
-        _check_forces(_np(F), Fo, pe, peo)
+        _check_forces(_np(F), Fo, pe, peo, _alts(orc, x, is_p, L, _oparams(orc, p)))
         e = _np(sim.particle_energies())
         assert np.abs(e - eo).max() <= 2e-6 * np.abs(eo).max()
         ke, pe2 = sim.energy()
@@ -132,7 +157,7 @@ def test_forces_mid_sizes(orc, N, density, r_c, k, Y_P, variant):
     with _sim_from_arrays(x, v, is_p, L, r_c=r_c, cell_subdiv=k, force_variant=variant) as sim:
         F, pe = sim.forces()
         Fo, eo, peo, d = orc.forces(x, is_p, L, _oparams(orc, sim.params))
-        _check_forces(_np(F), Fo, pe, peo)
+        _check_forces(_np(F), Fo, pe, peo, _alts(orc, x, is_p, L, _oparams(orc, sim.params)))
         cid, start, nc = sim.cells()
         cid_o, start_o = orc.cells(x, L, nc)
         assert np.array_equal(_np(cid), cid_o) and np.array_equal(_np(start), start_o)
@@ -146,7 +171,7 @@ def test_forces_clustered_occupancy(orc, variant):
     with _sim_from_arrays(x, v, is_p, L, T=0.75, force_variant=variant) as sim:
         F, pe = sim.forces()
         Fo, eo, peo, d = orc.forces(x, is_p, L, _oparams(orc, sim.params))
-        _check_forces(_np(F), Fo, pe, peo)
+        _check_forces(_np(F), Fo, pe, peo, _alts(orc, x, is_p, L, _oparams(orc, sim.params)))
 
 
 @pytest.mark.parametrize("variant", [0, 1])
@@ -311,10 +336,7 @@ def test_full_size_sampled_targets(orc, cfg):
         rng = np.random.default_rng(cfg)
         t = np.sort(rng.choice(c["N"], size=96 if cfg == 4 else 256, replace=False))
         Fo, eo, _, d = orc.forces(x, is_p, L, _oparams(orc, p), targets=t)
-        dF = F[t] - Fo
-        assert np.linalg.norm(dF) / np.linalg.norm(Fo) <= FORCE_TOL
-        frms = math.sqrt((np.linalg.norm(Fo, axis=1) ** 2).mean())
-        assert (np.linalg.norm(dF, axis=1) / np.maximum(np.linalg.norm(Fo, axis=1), frms)).max() <= FORCE_TOL
+        _check_forces(F[t], Fo, alternates=_alts(orc, x, is_p, L, _oparams(orc, p), t))
         assert abs(e[t].sum() - eo.sum()) <= PE_TOL * abs(eo.sum()) * 3
         assert e.sum() == pytest.approx(pe, rel=1e-12)
         assert np.abs(F.sum(0)).max() <= 1e-6 * np.abs(F).sum()          # Newton's third law
@@ -342,7 +364,7 @@ def test_exact_zero_skipping_changes_nothing_that_matters(orc, N, density, r_c, 
                 pairs, nonzero = sim.pair_counts()
     Fo, _, peo, d = orc.forces(x, is_p, L, orc.Params(r_c=r_c))
     for F, pe in res:
-        _check_forces(F, Fo, pe, peo)
+        _check_forces(F, Fo, pe, peo, _alts(orc, x, is_p, L, orc.Params(r_c=r_c)))
     assert np.linalg.norm(res[0][0] - res[1][0]) <= 2e-6 * np.linalg.norm(Fo)
     assert abs(res[0][1] - res[1][1]) <= 1e-7 * abs(peo)
     # the counters: in-range pairs as the oracle counts them (a pair within 1e-5 of r_c may flip, D22); the
@@ -378,7 +400,7 @@ def test_evolved_clustered_state_snapshots(orc, cfg, nsteps, nsample):
         F, e = _np(F), _np(sim.particle_energies())
         t = np.sort(np.random.default_rng(cfg).choice(c["N"], size=nsample, replace=False))
         Fo, eo, _, _ = orc.forces(x, is_p, L, _oparams(orc, p), targets=t)
-        _check_forces(F[t], Fo)
+        _check_forces(F[t], Fo, alternates=_alts(orc, x, is_p, L, _oparams(orc, p), t))
         assert abs(e[t].sum() - eo.sum()) <= 3 * PE_TOL * abs(eo.sum())
         ke, _ = sim.energy()
         assert ke == pytest.approx(1.5 * c["N"] * c["T"], rel=1e-9)        # rescaled every 10 steps (D7, D8)
@@ -401,7 +423,7 @@ def test_range_split_mode(orc, N, density, r_c, Y_P, variant):
         F, pe = sim.forces()
         pairs, nonzero = sim.pair_counts()
     Fo, _, peo, d = orc.forces(x, is_p, L, orc.Params(r_c=r_c, r_nuc=11.5))
-    _check_forces(_np(F), Fo, pe, peo)
+    _check_forces(_np(F), Fo, pe, peo, _alts(orc, x, is_p, L, orc.Params(r_c=r_c, r_nuc=11.5)))
     assert abs(pairs - d["ordered_pairs"]) <= 4 and nonzero < pairs
     with pytest.raises(pasta.PastaError):
         pasta.Sim(N, Y_P, density, 1.0, params=pasta.default_params(r_c=r_c, r_nuc=r_c + 1.0), seed=1)
