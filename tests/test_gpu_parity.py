@@ -466,3 +466,28 @@ def test_linear_box_only_expansion_mode(orc):
     assert np.abs(vg - vo).max() <= 1e-5  # 1e-4 fm over 40 fm/c of a chaotic trajectory
     with pytest.raises(pasta.PastaError):
         pasta.Sim(2048, 0.3, 0.05, 1.0, params=pasta.default_params(r_c=17.0, xi_dot=1e-5, scale_per_step=1.0001), seed=1)
+
+
+@pytest.mark.parametrize("seed", list(range(24)))
+def test_random_small_systems(orc, seed):
+    """Seeded sweep over sizes, proton fractions, densities and cut-offs (dense and sparse chunk builders, one to
+    dozens of cells per side, boxes barely wider than 2 r_c, single-species systems): forces and PE against the
+    oracle, uniform and clustered positions."""
+    rng = np.random.default_rng(1000 + seed)
+    N = int(rng.integers(1, 3000))
+    Y_P = float(rng.choice([0.0, 0.05, 0.3, 0.5, 1.0]))
+    density = float(10 ** rng.uniform(-3.3, -0.9))
+    L = inputs.box_length(N, density)
+    r_c = float(min(rng.uniform(4.0, 20.0), 0.499 * L))
+    gen = inputs.clustered_state if (seed % 3 == 0 and N > 200) else inputs.uniform_state
+    x, v, is_p, L = gen(N, Y_P, density, 1.0, seed=seed)
+    with _sim_from_arrays(x, v, is_p, L, r_c=r_c) as sim:
+        F, pe = sim.forces()
+        pairs = sim.pair_count()
+    op = orc.Params(r_c=r_c)
+    Fo, _, peo, d = orc.forces(x, is_p, L, op)
+    if np.linalg.norm(Fo) > 0:
+        _check_forces(_np(F), Fo, pe, peo if abs(peo) > 1e-9 else None, _alts(orc, x, is_p, L, op))
+    else:
+        assert np.abs(_np(F)).max() == 0.0
+    assert abs(pairs - d["ordered_pairs"]) <= 4
