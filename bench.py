@@ -132,7 +132,7 @@ def run_reference(args, rank, world):
         return
     c = inputs.CONFIGS[args.config]
     total = max(1, args.steps + args.warmup)
-    per_step = min(8.0, 150.0 / total)
+    per_step = min(8.0, 90.0 / total)
     vals = []
     base = None
     state = inputs.config_state(args.config, 1)
