@@ -204,7 +204,7 @@ def run_ours(args, rank, world, local_rank):
     for kv in filter(None, args.params.split(",")):  # tuning overrides, e.g. --params x_subdiv=8,auto_grid=0
         key, val = kv.split("=")
         setattr(prm, key, type(getattr(prm, key))(float(val)))
-    sim = pasta.Sim(N, c["Y_P"], c["density"], c["T"], params=prm, seed=1 + rank)
+    sim = pasta.Sim(N, c["Y_P"], c["density"], c["T"], params=prm, seed=args.seed + rank)
     flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")
 
     def barrier():
@@ -377,6 +377,7 @@ def main():
     ap.add_argument("--sweep", type=int, default=0, choices=[0, 3, 5],
                     help="run the whole decompression of config 3 or 5 and report steps/s against density")
     ap.add_argument("--sweep-chunk", type=int, default=1000)
+    ap.add_argument("--seed", type=int, default=1, help="seed of the synthetic start (rank r uses seed + r)")
     ap.add_argument("--params", default="", help="comma-separated pasta_params overrides (tuning experiments)")
     ap.add_argument("--cpu-budget", type=float, default=15.0, help="seconds of oracle time for cpu_baseline")
     ap.add_argument("--no-cpu-baseline", action="store_true")
