@@ -74,6 +74,7 @@ struct ChunkArgs {
   const int32_t* chunk_tab;  // [chunk][8] sorted slots of the chunk's targets, -1 = none (k1_cells.cu)
   const int32_t* counts;     // [0] number of chunks in the overflow region
   int32_t nprim;             // primary entries (some of them empty)
+  int32_t merged;            // the two species' grids are identical: neutron chunks take both in one pass
   SpeciesGrid g[2];
   float rcS;     // sigma * r_c
   float rnS;     // sigma * r_n (cut-off of the nuclear terms)
@@ -99,6 +100,7 @@ struct WarpShared {
   float4 tile[2][32];
   float4 seg[SEG_CAP + 1];
   int cum[SEG_CAP + 1 + 32];
+  float flag[SEG_CAP + 1];  // BOTH-species streams: 0 = the segment holds protons, 1 = neutrons
 };
 
 // A lane's packed pair of targets (minus their coordinates) and its partial sums.
@@ -111,12 +113,15 @@ struct Accum {
 };
 struct PassConsts {
   float g2a, gB, a, B;
+  float gB_n, B_n;  // BOTH-species streams: gB, B apply to proton sources, gB_n, B_n to neutron sources
 };
 
 // One source against the lane's two targets.
-template <bool COUL, bool CUT, bool ENERGY>
+template <bool COUL, bool CUT, bool ENERGY, bool BOTH>
 __device__ __forceinline__ void evaluate(const float4 s, const Targets& t, Accum& acc, const PassConsts& k,
                                          const PairConsts& c) {
+  // BOTH: the stream mixes the two source species; s.w tells which, and with it the isospin constants
+  const float gB = BOTH ? (s.w != 0.f ? k.gB_n : k.gB) : k.gB, B = BOTH ? (s.w != 0.f ? k.B_n : k.B) : k.B;
   const float2 dx = __fadd2_rn(dup(s.x), t.ntx);
   const float2 dy = __fadd2_rn(dup(s.y), t.nty);
   const float2 dz = __fadd2_rn(dup(s.z), t.ntz);
@@ -129,8 +134,8 @@ __device__ __forceinline__ void evaluate(const float4 s, const Targets& t, Accum
     u.x = nr2.x > -c.rn2s ? u.x : 0.f;
     u.y = nr2.y > -c.rn2s ? u.y : 0.f;
   }
-  float2 g = __fmul2_rn(u, __ffma2_rn(dup(k.g2a), u, dup(k.gB)));
-  if (ENERGY) acc.e = __ffma2_rn(u, __ffma2_rn(dup(k.a), u, dup(k.B)), acc.e);
+  float2 g = __fmul2_rn(u, __ffma2_rn(dup(k.g2a), u, dup(gB)));
+  if (ENERGY) acc.e = __ffma2_rn(u, __ffma2_rn(dup(k.a), u, dup(B)), acc.e);
   if (COUL) {
     // screened Coulomb, cut at r_c, skipped at r = 0 (the self pair and coincident protons, D2):
     // 1/r' := 0 for excluded pairs, which zeroes every Coulomb factor without creating inf * 0
@@ -167,10 +172,12 @@ struct Cursor {
   int cur;     // segment index
   int end;     // stream position at which segment `cur` ends
   float4 rec;  // its record
+  float flag;  // BOTH-species streams: its species flag
 };
 
 // Raw source of stream position `pos` for this lane (zeros past the end of the stream) and the record of the
 // segment it belongs to.  A lane's positions grow by 32 per tile, so the cursor only ever moves forward.
+template <bool BOTH>
 __device__ __forceinline__ void fetch(const ChunkArgs& A, const WarpShared& sh, Cursor& cu, const int pos,
                                       const int total, float4& q, float4& m) {
   if (pos >= cu.end) {
@@ -179,19 +186,22 @@ __device__ __forceinline__ void fetch(const ChunkArgs& A, const WarpShared& sh, 
       cu.end = sh.cum[cu.cur + 1];
     } while (pos >= cu.end);
     cu.rec = sh.seg[cu.cur];
+    if (BOTH) cu.flag = sh.flag[cu.cur];
   }
   m = cu.rec;
   q = make_float4(0.f, 0.f, 0.f, 0.f);
   if (pos < total) q = __ldg(A.pos4 + (__float_as_int(cu.rec.x) + pos));
+  if (BOTH) m.x = cu.flag;  // the slot offset has served; its place carries the species flag to to_frame
 }
 
 // source position in the frame: cell-relative coordinate + integer cell offset * cell width
+template <bool BOTH>
 __device__ __forceinline__ float4 to_frame(const float4 q, const float4 m, const float wxS) {
   float4 s;
   s.x = fmaf(q.w + m.y, wxS, q.x);
   s.y = __fadd_rn(q.y, m.z);
   s.z = __fadd_rn(q.z, m.w);
-  s.w = 0.f;
+  s.w = BOTH ? m.x : 0.f;
   return s;
 }
 
@@ -200,7 +210,7 @@ __device__ __forceinline__ float4 to_frame(const float4 q, const float4 m, const
 // one into the chunk's frame and stores it in the shared double buffer.  Consumer: every lane evaluates
 // STEPS sources of the tile against its pair of targets.  Positions past the end of the stream become idle
 // sources ~1e11 away, which contribute exact zeros.
-template <bool COUL, bool CUT, bool ENERGY, bool STATS>
+template <bool COUL, bool CUT, bool ENERGY, bool STATS, bool BOTH>
 __device__ __forceinline__ void run_stream(const ChunkArgs& A, const PairConsts& c, WarpShared& sh, const int lane,
                                            const int total, const float wxS, const Targets& t, Accum& acc,
                                            const PassConsts& k, unsigned long long* st) {
@@ -211,18 +221,19 @@ __device__ __forceinline__ void run_stream(const ChunkArgs& A, const PairConsts&
   cu.cur = 0;
   cu.end = sh.cum[1];
   cu.rec = sh.seg[0];
+  cu.flag = BOTH ? sh.flag[0] : 0.f;
   float4 q, m;
-  fetch(A, sh, cu, lane, total, q, m);
+  fetch<BOTH>(A, sh, cu, lane, total, q, m);
   float4* const wr = &sh.tile[0][lane];
   const float4* const rd = &sh.tile[0][ph];
 #pragma unroll 1
   for (int i = 0; i < ntile; ++i) {
     const int o = (i & 1) * 32;
-    wr[o] = to_frame(q, m, wxS);
-    fetch(A, sh, cu, ((i + 1) << 5) + lane, total, q, m);
+    wr[o] = to_frame<BOTH>(q, m, wxS);
+    fetch<BOTH>(A, sh, cu, ((i + 1) << 5) + lane, total, q, m);
     __syncwarp();
 #pragma unroll
-    for (int j = 0; j < STEPS; ++j) evaluate<COUL, CUT, ENERGY>(rd[o + NPH * j], t, acc, k, c);
+    for (int j = 0; j < STEPS; ++j) evaluate<COUL, CUT, ENERGY, BOTH>(rd[o + NPH * j], t, acc, k, c);
   }
   __syncwarp();
   if (STATS && lane == 0) {
@@ -239,7 +250,9 @@ struct Box {
 
 // One pass of a chunk over one source species: list the segments (lanes run over the rows of the source
 // grid), stream them whenever the list is full and at the end.
-template <bool COUL, bool CUT, bool ENERGY, bool STATS>
+// BOTH: the two species share one grid geometry (gs = either) and the pass lists the segments of both, every row
+// once: a "round" is then a (periodic image, species) pair.
+template <bool COUL, bool CUT, bool ENERGY, bool STATS, bool BOTH>
 __device__ __forceinline__ void source_pass(const ChunkArgs& A, const PairConsts& c, WarpShared& sh, const int lane,
                                             const SpeciesGrid& gs, const int rx, const int ry, const int rz,
                                             const Box& b, const Targets& t, Accum& acc, const PassConsts& k,
@@ -283,7 +296,7 @@ __device__ __forceinline__ void source_pass(const ChunkArgs& A, const PairConsts
             ax_lo = rx + (int)floorf((b.lo_x - xr) * gs.inv_wxS + 0.5f);
             ax_hi = rx + (int)floorf((b.hi_x + xr) * gs.inv_wxS + 0.5f);
             q_lo = floor_div(ax_lo, ncx);
-            nseg = floor_div(ax_hi, ncx) - q_lo + 1;
+            nseg = (floor_div(ax_hi, ncx) - q_lo + 1) * (BOTH ? 2 : 1);
             const int ay = wrap_cell(ry + my, nc), az = wrap_cell(rz + mz, nc);
             rowbase = gs.base + (az * nc + ay) * ncx;
           }
@@ -291,11 +304,13 @@ __device__ __forceinline__ void source_pass(const ChunkArgs& A, const PairConsts
       }
       int start = 0, len = 0;
       float xoff = 0.f;
+      const int spi = BOTH ? (round & 1) : 0;  // BOTH: species of this round's segments
       if (round < nseg) {
-        const int q = q_lo + round, qb = q * ncx;
+        const int q = q_lo + (BOTH ? round >> 1 : round), qb = q * ncx;
         const int a_lo = max(ax_lo, qb) - qb, a_hi = min(ax_hi, qb + ncx - 1) - qb;
-        start = __ldg(A.bin_start + rowbase + a_lo);
-        len = __ldg(A.bin_start + rowbase + a_hi + 1) - start;
+        const int rb = rowbase + (BOTH ? A.g[spi].base - gs.base : 0);
+        start = __ldg(A.bin_start + rb + a_lo);
+        len = __ldg(A.bin_start + rb + a_hi + 1) - start;
         xoff = (float)(qb - rx);
       }
       // append the non-empty segments in lane order; stream positions by an inclusive scan of the lengths
@@ -310,6 +325,7 @@ __device__ __forceinline__ void source_pass(const ChunkArgs& A, const PairConsts
         const int at = nseg_list + __popc(has & lt_mask), begin = total + incl - len;
         sh.seg[at] = make_float4(__int_as_float(start - begin), xoff, yoff, zoff);
         sh.cum[at] = begin;
+        if (BOTH) sh.flag[at] = (float)spi;
       }
       nseg_list += __popc(has);
       total += __shfl_sync(0xffffffffu, incl, 31);
@@ -320,11 +336,14 @@ __device__ __forceinline__ void source_pass(const ChunkArgs& A, const PairConsts
       }
     }
     // close the list (dummy record for idle lanes, +infinity boundaries) and stream it
-    if (lane == 0) sh.seg[nseg_list] = make_float4(0.f, XOFF_IDLE, 0.f, 0.f);
+    if (lane == 0) {
+      sh.seg[nseg_list] = make_float4(0.f, XOFF_IDLE, 0.f, 0.f);
+      if (BOTH) sh.flag[nseg_list] = 0.f;
+    }
     sh.cum[nseg_list + lane] = lane == 0 ? total : 0x3fffffff;
     if (lane == 0) sh.cum[nseg_list + 32] = 0x3fffffff;
     __syncwarp();
-    run_stream<COUL, CUT, ENERGY, STATS>(A, c, sh, lane, total, gs.wxS, t, acc, k, st);
+    run_stream<COUL, CUT, ENERGY, STATS, BOTH>(A, c, sh, lane, total, gs.wxS, t, acc, k, st);
   } while (rbase < nrows);
 }
 
@@ -339,7 +358,9 @@ __device__ __forceinline__ int min_image_cells(int m, int nc) {
 // a small block of cells instead.  Compact chunks keep the bounding box tight (few wasted candidates) and the
 // frame coordinates small (FP32 ulp of a displacement <= 1e-6 fm).  The frame's origin cell is the middle of the
 // targets' cell range.
-template <bool CUT, bool ENERGY, bool STATS>
+// MERGE: on identical grids a neutron chunk takes both source species in ONE pass (one listing instead of two: it
+// is the listing, not the arithmetic, that a sparse system pays for).
+template <bool CUT, bool ENERGY, bool STATS, bool MERGE>
 __device__ __forceinline__ void chunk_passes(const ChunkArgs& A, const PairConsts& c, WarpShared& sh, const int lane,
                                              const int pr, const SpeciesGrid& gt, const int st_sp, const bool chunk_p,
                                              const float4 tp, const int tc, const unsigned active, Accum& acc,
@@ -366,8 +387,10 @@ __device__ __forceinline__ void chunk_passes(const ChunkArgs& A, const PairConst
   oy += oy < 0 ? gt.ncell : 0;
   oz += oz < 0 ? gt.ncell : 0;
   // ---- pass 0: proton sources, pass 1: neutron sources -------------------------------------------------
+  const bool both = MERGE && A.merged != 0 && !chunk_p;
 #pragma unroll
   for (int sp = 0; sp < 2; ++sp) {
+    if (MERGE && both && sp == 0) continue;  // the neutron pass below lists the protons too
     const SpeciesGrid& gs = A.g[sp];
     // Frame of the pass: origin = centre of the source-grid cell (rx, ry, rz) that contains the centre of
     // the chunk's origin cell.  Same grid: identical arithmetic for targets and sources (a target meets
@@ -422,10 +445,17 @@ __device__ __forceinline__ void chunk_passes(const ChunkArgs& A, const PairConst
     k.gB = like ? c.gB_like : c.gB_unlike;
     k.a = c.a;
     k.B = like ? c.B_like : c.B_unlike;
-    if (sp == 0 && chunk_p)
-      source_pass<true, CUT, ENERGY, STATS>(A, c, sh, lane, gs, rx, ry, rz, b, t, acc, k, st);
-    else
-      source_pass<false, CUT, ENERGY, STATS>(A, c, sh, lane, gs, rx, ry, rz, b, t, acc, k, st);
+    k.gB_n = c.gB_like;  // (BOTH: neutron targets; proton sources are unlike, neutron sources like)
+    k.B_n = c.B_like;
+    if (MERGE && both) {
+      k.gB = c.gB_unlike;
+      k.B = c.B_unlike;
+      source_pass<false, CUT, ENERGY, STATS, true>(A, c, sh, lane, gs, rx, ry, rz, b, t, acc, k, st);
+    } else if (sp == 0 && chunk_p) {
+      source_pass<true, CUT, ENERGY, STATS, false>(A, c, sh, lane, gs, rx, ry, rz, b, t, acc, k, st);
+    } else {
+      source_pass<false, CUT, ENERGY, STATS, false>(A, c, sh, lane, gs, rx, ry, rz, b, t, acc, k, st);
+    }
   }
 }
 
@@ -463,7 +493,8 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) k2_chunk_kernel(const ChunkA
   acc.fx = acc.fy = acc.fz = acc.e = make_float2(0.f, 0.f);
   unsigned long long st[3] = {0, 0, 0};
 
-  chunk_passes<CUT, ENERGY, STATS>(A, c, sh, lane, pr, gt, st_sp, chunk_p, tp, tc, active, acc, st);
+  chunk_passes<CUT, ENERGY, STATS, MINB == K2_MINB_SPARSE>(A, c, sh, lane, pr, gt, st_sp, chunk_p, tp, tc, active, acc,
+                                                           st);
 
   // ---- combine the phases' FP32 partials in FP64 ------------------------------------------------------------
   // quantity index q = 4 * (target within the pair) + {fx, fy, fz, e}; a transposing butterfly over the
@@ -529,6 +560,7 @@ int k2_chunk_forces(Sim* s, bool with_energy, bool stats) {
   A.chunk_tab = s->chunk_tab.as<int32_t>();
   A.counts = s->counters.as<int32_t>() + 2 * 24;
   A.nprim = (int32_t)s->chunk_nprim;
+  A.merged = s->grid_sp[0].ncell == s->grid_sp[1].ncell && s->grid_sp[0].ncx == s->grid_sp[1].ncx ? 1 : 0;
   for (int sp = 0; sp < 2; ++sp) {
     const Grid& g = s->grid_sp[sp];
     A.g[sp].ncell = g.ncell;
