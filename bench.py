@@ -348,6 +348,9 @@ def run_sweep(args):
     comp = sim.composition(12)
     torch.cuda.synchronize()
     fof_s = time.perf_counter() - t0
+    # the paper's own two-radius MST clusters on the same final configuration
+    _, ncl_mst = sim.clusters_mst(4.5, 3.0)
+    comp_mst = sim.composition(12)
     A = A.cpu().numpy()
     Z = Z.cpu().numpy()
     heavy = A >= 12
@@ -358,7 +361,7 @@ def run_sweep(args):
         hist[(a_ // 20 * 20, z_ // 10 * 10)] = hist.get((a_ // 20 * 20, z_ // 10 * 10), 0) + 1
     line = {"sweep": args.sweep, "workload": workload_config(args.sweep, 1)["workload"] + ", decompression to 0.00125 fm^-3",
             "steps": c["steps"], "wall_s": wall, "points": pts, "clusters": ncl, "fof_s": fof_s, "composition": comp,
-            "largest_A": int(A.max()), "AZ_histogram_A20_Z10_bins": {"%d,%d" % k: v for k, v in sorted(hist.items())}}
+            "mst_r_pp_4.5_r_np_3.0": {"clusters": ncl_mst, "composition": comp_mst}, "largest_A": int(A.max()), "AZ_histogram_A20_Z10_bins": {"%d,%d" % k: v for k, v in sorted(hist.items())}}
     print(json.dumps(line), flush=True)
     sim.close()
 
