@@ -330,6 +330,9 @@ __global__ void k1_chunk_blocks_kernel(int sp, const int32_t* __restrict__ bin_s
 }
 
 // Cells per side of a species' grid: the O3 formula with the k that puts about CHUNK particles in a cell.
+#ifndef PASTA_WMAX
+#define PASTA_WMAX 8.0
+#endif
 static int auto_subdiv(double L, double r_c, int64_t n_species, int k_default) {
   if (n_species <= 0) return k_default;
   const double w_star = L * cbrt((double)PASTA_CHUNK_T / (double)n_species);
@@ -337,7 +340,7 @@ static int auto_subdiv(double L, double r_c, int64_t n_species, int k_default) {
   // never wider than 8 fm: sorted coordinates are FP32 offsets from the cell centre, and their quantum
   // (2^-24 of the half width) times the steepest pair-force gradient (~80 MeV/fm^2 inside a cluster) has to
   // stay below the force tolerance
-  const int k_min = (int)ceil(r_c / 8.0);
+  const int k_min = (int)ceil(r_c / PASTA_WMAX);
   k = k < k_min ? k_min : k;
   return k < 1 ? 1 : (k > 64 ? 64 : k);
 }
