@@ -8,6 +8,7 @@ package imports nothing from there.  Allowed callers: ``tests/``, ``__graft_entr
 from .pasta_oracle import (  # noqa: F401
     Params,
     build,
+    cell_coords,
     cells,
     clusters,
     clusters_cells,

@@ -180,6 +180,22 @@ void orc_cells(int64_t N, const double* x, double L, int32_t ncell, int32_t* cel
 }
 
 /*
+ * O3 per axis: c = min(n-1, (int)floor(x (n / L))) for every coordinate of x (3N of them), the
+ * statement inside orc_cells above written out on its own, so that a grid with different cell
+ * counts per axis (the force path's thin cells along x: n = ncx for x, n = ncell for y, z) can be
+ * checked without allocating an n^3 table (reading D14).
+ */
+void orc_cell_coords(int64_t N3, const double* x, double L, int32_t n, int32_t* c) {
+  const double inv_w = (double)n / L;
+  for (int64_t k = 0; k < N3; ++k) {
+    int32_t q = (int32_t)floor(x[k] * inv_w);
+    if (q > n - 1) q = n - 1;
+    if (q < 0) q = 0;
+    c[k] = q;
+  }
+}
+
+/*
  * P7 helper: the same force definition evaluated through the O3 cell grid (own + 26
  * neighbour cells) -- an independent pair enumeration used to pin orc_forces
  * against itself on tiny N and as the labelled "list-based" second CPU baseline.

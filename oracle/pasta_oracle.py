@@ -142,6 +142,16 @@ def cells(x, L, n_cell):
     return cid, start
 
 
+def cell_coords(x, L, n):
+    """O3 per axis: c = min(n-1, floor(x n / L)) for every coordinate; returns int32 array of x's shape."""
+    x = _f64(x)
+    c = np.zeros(x.shape, dtype=np.int32)
+    lib = _load()
+    lib.orc_cell_coords.restype = None
+    lib.orc_cell_coords(C.c_int64(x.size), _p(x), C.c_double(L), C.c_int32(n), _p(c))
+    return c
+
+
 def kinetic(v, mass):
     v = _f64(v, (-1, 3))
     return float(_load().orc_kinetic(C.c_int64(v.shape[0]), _p(v), C.c_double(mass)))

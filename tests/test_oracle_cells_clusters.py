@@ -37,6 +37,27 @@ def test_cells_faces_and_clamp(orc):
     assert orc.ncell(5.0, 20.0, 1) == 1  # max(1, .)
 
 
+def test_cell_coords_per_axis_is_the_o3_statement(orc):
+    """orc.cell_coords (O3 per axis, used to check the force path's anisotropic grids) against what pins O3
+    itself: the ids of orc.cells decoded axis by axis, the face/clamp hand cases above, and the interval property."""
+    x, v, is_p, L = inputs.uniform_state(3000, 0.3, 0.05, 1.0, seed=4)
+    for nc in (1, 2, 5, 13):
+        cid, _ = orc.cells(x, L, nc)
+        c = orc.cell_coords(x, L, nc)
+        assert c.shape == x.shape and c.dtype == np.int32
+        assert np.array_equal(c[:, 0], cid % nc) and np.array_equal(c[:, 1], (cid // nc) % nc)
+        assert np.array_equal(c[:, 2], cid // (nc * nc))
+    hand = np.array([[0.0, 3.0, 6.0], [9.0, 11.999999999999998, 2.9999999999999996], [3.0, 3.0, 3.0]])
+    assert orc.cell_coords(hand, 12.0, 4).tolist() == [[0, 1, 2], [3, 3, 0], [1, 1, 1]]
+    # a different cell count for one axis (thin cells along x): intervals [c w, (c+1) w) with w = L / n
+    n = 37
+    c = orc.cell_coords(x[:, 0], L, n)
+    w = L / n
+    assert c.min() == 0 and c.max() == n - 1
+    assert (c * w <= x[:, 0] + 1e-12).all() and (x[:, 0] < (c + 1) * w + 1e-12).all()
+    assert orc.cell_coords(np.array([L * (1 - 1e-17), -0.0]), L, n).tolist() == [n - 1, 0]  # clamp, as orc_cells
+
+
 def _chain(n, spacing, start, axis=0):
     x = np.tile(np.asarray(start, dtype=float), (n, 1))
     x[:, axis] += spacing * np.arange(n)

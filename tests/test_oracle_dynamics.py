@@ -85,6 +85,19 @@ def test_time_reversibility(orc):
     assert np.abs(v2 + v).max() < 1e-11
 
 
+def test_kinetic_energy_hand_values(orc):
+    """orc_kinetic = sum 1/2 M |v|^2 against values worked by hand, so that the prefactor is pinned by
+    something other than the thermostat that uses it: one nucleon at v = (0.1, 0, 0) c carries 1/2 939 0.01 = 4.695 MeV;
+    components add in quadrature; particles add."""
+    assert orc.kinetic(np.array([[0.1, 0.0, 0.0]]), 939.0) == pytest.approx(4.695, rel=1e-15)
+    assert orc.kinetic(np.array([[0.3, -0.4, 0.0]]), 2.0) == pytest.approx(0.25, rel=1e-15)
+    assert orc.kinetic(np.array([[0.1, 0, 0], [0, 0.2, 0], [0, 0, -0.2]]), 100.0) == pytest.approx(0.5 + 2.0 + 2.0, rel=1e-15)
+    assert orc.kinetic(np.zeros((5, 3)), 939.0) == 0.0
+    # and the thermostat target of PAPER.md:110: mean KE per particle 3/2 T  <=>  KE = 3/2 N T
+    v = np.full((1000, 3), math.sqrt(0.75 / 939.0))
+    assert orc.kinetic(v, 939.0) == pytest.approx(1.5 * 1000 * 0.75, rel=1e-14)
+
+
 def test_p9_thermostat(orc):
     """After a rescale step sum 1/2 M v^2 = (3/2) N T exactly; only on steps whose
     1-based count is a multiple of the interval, counter persisting across calls (D7)."""

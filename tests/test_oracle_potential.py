@@ -43,6 +43,36 @@ def test_p1_two_particle_table(orc):
     assert n == 9
 
 
+def test_p1_table_regenerated_in_long_double():
+    """the stored table (the surveyor's evaluation) regenerated here, independently of the oracle, by
+    writing Eq. 1a-c with the constants of Table I, alpha hbar c = 1.44 MeV fm and
+    lambda = 10 fm in x87 extended precision (numpy.longdouble, 64-bit mantissa) -- V as printed in the
+    paper, F = -dV/dr differentiated by hand term by term.  Two independent evaluations of the paper's formula must
+    agree to the digits the table prints."""
+    ld = np.longdouble
+    if np.finfo(ld).nmant < 63:
+        pytest.skip("numpy.longdouble is not the x87 extended type on this host")
+    a, b, c, Lam, alpha, lam = ld(110), ld(-26), ld(24), ld(5) / ld(4), ld(144) / ld(100), ld(10)
+    n = 0
+    for line in open(os.path.join(GOLD, "two_particle_table.txt")):
+        if line.startswith("#") or not line.strip():
+            continue
+        kind, r, V, F = line.split()
+        r = ld(r)
+        B = b - c if kind == "np" else b + c                     # Eq. 1a vs 1b/1c: the sign of c by isospin
+        g1, g2 = np.exp(-r * r / Lam), np.exp(-r * r / (2 * Lam))
+        v = a * g1 + B * g2                                       # a e^{-r^2/Lambda} + (b -+ c) e^{-r^2/2 Lambda}
+        f = (2 * r / Lam) * a * g1 + (r / Lam) * B * g2           # -d/dr of the two Gaussians
+        if kind == "pp":
+            y = alpha * np.exp(-r / lam) / r                      # Eq. 1c: + alpha e^{-r/lambda} / r
+            v, f = v + y, f + y * (1 / r + 1 / lam)
+        assert float(v) == pytest.approx(float(V), rel=1e-4 if float(r) > 11 else 2e-9), (kind, r)
+        if F != "nan":
+            assert float(f) == pytest.approx(float(F), rel=2e-9), (kind, r)
+        n += 1
+    assert n == 9
+
+
 def test_p1_pair_in_box_matches_isolated_pair(orc):
     """The N-body sum for N = 2 in a big periodic box reproduces the table: force direction (repulsive
     at 1 fm pushes i away from j), the factor 1/2 in e_i, PE = V."""
