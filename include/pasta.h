@@ -53,16 +53,18 @@ typedef struct pasta_params {
   double mass;                 /* nucleon mass M = 939 MeV */
   double scale_per_step;       /* s: each pasta_step multiplies L and x by s in the drift (D9, D10); 1 = fixed box */
   int32_t thermostat_interval; /* rescale |v| so that KE = 3/2 N T after every k-th step (D7, D8); 0 = off */
-  int32_t cell_subdiv;         /* k >= 1: cells per side = max(1, floor(L k / r_c)), width L/ncell >= r_c/k (D14) */
-  int32_t force_variant;       /* 0 = library default; >0 selects a specific pair-force kernel */
+  int32_t cell_subdiv;         /* k >= 1 of the grid pasta_cells reports: cells per side = max(1, floor(L k / r_c)),
+                                  width L/ncell >= r_c/k (D14).  (The force path sizes its own per-species grids with the
+                                  same formula: pasta_force_grid / pasta_force_cells.) */
   int32_t energy_every_step;   /* 1 (default): pasta_step evaluates per-particle energies with the forces */
-  int32_t auto_grid;           /* 1 (default): each species' force grid picks its own k (about 8 particles per cell);
-                                  0: both use cell_subdiv.  pasta_cells always reports the cell_subdiv grid */
-  int32_t x_subdiv;            /* thin cells along x per force-grid cell (0 = library default: 8, fewer for a sparse species) */
   int32_t skip_exact_zeros;    /* 1 (default): np/nn candidates beyond the distance at which exp2(-r^2 log2e/2 Lambda)
                                   underflows FP32 (14.78 fm for Lambda = 1.25) are not streamed: their terms are exactly
                                   0.0f in the kernel's arithmetic, so F and e are unchanged (D23).  0: stream to r_c */
-  int32_t reserved1;
+  int32_t list_reuse;          /* 1 (default): where a species is sparse the sorted order, the chunk table and every chunk's
+                                  source-segment list are built with a halo (skin) and kept across steps until some particle
+                                  has moved more than half the halo -- the paper's neighbour list with its displacement
+                                  trigger.  F and e do not depend on it.  0: rebuild every step */
+  double list_halo;            /* halo thickness delta_r in fm (4 fm); 0 = library default */
   double r_nuc;                /* > 0: the paper's own range split: the nuclear (Gaussian) terms are zero
                                   and not computed beyond r_nuc (11.5 fm in the paper) while the Coulomb term still reaches
                                   r_c.  0 (default): one cut-off r_c for every term (D1).  Must be <= r_c */
@@ -95,7 +97,7 @@ int pasta_params_default(pasta_params* p);
  * from `seed` by a counter-based generator: positions uniform in [0,L)^3, velocity components normal
  * with variance T/M (D15).  T is also the thermostat target.  env may be NULL (device 0,
  * default stream, cudaMalloc).
- * EINVAL: out/p NULL, wrong struct_size, N <= 0 or N > 2^30, Y_P outside [0,1], density <= 0, T < 0,
+ * EINVAL: out/p NULL, wrong struct_size, N <= 0 or N >= 2^26 (sorted slots are packed in 26 bits), Y_P outside [0,1], density <= 0, T < 0,
  * r_c <= 0, r_c > L/2 (the nearest image would be ambiguous; D3), Lambda/lambda/mass <= 0,
  * scale_per_step <= 0, thermostat_interval < 0, cell_subdiv < 1.
  */
@@ -164,13 +166,29 @@ int pasta_set_state_host(pasta_sim* sim, const double* x_host, const double* v_h
                          const double* F_host, double L);
 
 /*
- * Cell assignment of the current positions on the force grid (D14):
+ * Cell assignment of the current positions on the species-independent grid of pasta_params.cell_subdiv
+ * (D14) -- NOT the grids the force kernel sorts on, see pasta_force_cells below:
  *   ncell = max(1, floor(L k / r_c)); c = min(ncell-1, floor(x * (ncell/L))) per axis (FP64);
  *   id = (cz ncell + cy) ncell + cx;  cell_start = exclusive prefix sum of the histogram of id.
  * cell_id_dev [N], cell_start_dev [ncell^3 + 1] (size it with pasta_ncell first), either may be NULL.
  */
 int pasta_cells(pasta_sim* sim, int32_t* cell_id_dev, int32_t* cell_start_dev, int32_t* ncell_side_host);
 int pasta_ncell(pasta_sim* sim, int32_t* ncell_side_host); /* no device work */
+
+/*
+ * The cell lists the pair-force kernel really runs on (D14 applied per species).
+ * Each species has its own grid: ncell cells per side in y and z, ncx = ncell * (thin cells per cell) along x, both
+ * from the O3 formula c = min(n-1, floor(x * (n/L))) in FP64 with n = ncx for x and n = ncell for y, z.
+ *   pasta_force_grid:  out4_host = {ncell_p, ncx_p, ncell_n, ncx_n} for the current box (no device work).
+ *   pasta_force_cells: rebuilds the list for the CURRENT positions and copies it out:
+ *     bin_dev [N]            bin of particle i (original order) = base_s + (cz ncell_s + cy) ncx_s + cx,
+ *                            base_p = 0, base_n = ncell_p^2 ncx_p (protons' bins first);
+ *     bin_start_dev [B + 1]  exclusive prefix sum of the histogram of bin, B = ncell_p^2 ncx_p + ncell_n^2 ncx_n;
+ *     perm_dev [N]           sorted slot -> original index, ascending index inside a bin (a stable counting sort).
+ *   Any pointer may be NULL.  Asynchronous.
+ */
+int pasta_force_grid(pasta_sim* sim, int32_t* out4_host);
+int pasta_force_cells(pasta_sim* sim, int32_t* bin_dev, int32_t* bin_start_dev, int32_t* perm_dev);
 
 /* KE = sum 1/2 M v^2 and PE of the current state (forces re-evaluated if stale).  Synchronises. */
 int pasta_energy(pasta_sim* sim, double* ke_host, double* pe_host);
@@ -188,6 +206,8 @@ int pasta_pair_counts(pasta_sim* sim, int64_t* out2_host);
  * rows (summed over chunks), tiles of <= 32 sources, pair evaluations executed}.  Synchronises.
  * (ordered in-range pairs / pair evaluations = the kernel's useful-work fraction.) */
 int pasta_force_stats(pasta_sim* sim, int64_t* out3_host);
+/* Neighbour-list bookkeeping (list_reuse): out2_host = {force evaluations so far, of which rebuilt the list}. */
+int pasta_list_stats(pasta_sim* sim, int64_t* out2_host);
 
 /*
  * Instrumentation.  pasta_set_timing(sim, 1) brackets the cell-list, pair-force and integrate kernels

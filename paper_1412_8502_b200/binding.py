@@ -27,10 +27,9 @@ class Params(C.Structure):
         ("a", C.c_double), ("b", C.c_double), ("c", C.c_double), ("Lambda", C.c_double),
         ("alpha_hbarc", C.c_double), ("lambda_", C.c_double), ("r_c", C.c_double), ("mass", C.c_double),
         ("scale_per_step", C.c_double),
-        ("thermostat_interval", C.c_int32), ("cell_subdiv", C.c_int32), ("force_variant", C.c_int32),
-        ("energy_every_step", C.c_int32), ("auto_grid", C.c_int32), ("x_subdiv", C.c_int32),
-        ("skip_exact_zeros", C.c_int32), ("reserved1", C.c_int32),
-        ("r_nuc", C.c_double), ("xi_dot", C.c_double),
+        ("thermostat_interval", C.c_int32), ("cell_subdiv", C.c_int32), ("energy_every_step", C.c_int32),
+        ("skip_exact_zeros", C.c_int32), ("list_reuse", C.c_int32),
+        ("list_halo", C.c_double), ("r_nuc", C.c_double), ("xi_dot", C.c_double),
     ]
 
 
@@ -64,6 +63,9 @@ SIGNATURES = {
     "pasta_set_state_host": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_double]),
     "pasta_cells": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.POINTER(C.c_int32)]),
     "pasta_ncell": (C.c_int, [C.c_void_p, C.POINTER(C.c_int32)]),
+    "pasta_force_grid": (C.c_int, [C.c_void_p, C.POINTER(C.c_int32)]),
+    "pasta_force_cells": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]),
+    "pasta_list_stats": (C.c_int, [C.c_void_p, C.POINTER(C.c_int64)]),
     "pasta_energy": (C.c_int, [C.c_void_p, C.POINTER(C.c_double), C.POINTER(C.c_double)]),
     "pasta_particle_energies": (C.c_int, [C.c_void_p, C.c_void_p]),
     "pasta_pair_count": (C.c_int, [C.c_void_p, C.POINTER(C.c_int64)]),
@@ -290,6 +292,27 @@ class Sim:
         _check(self.lib.pasta_cells(self._h, C.c_void_p(cid.data_ptr()), C.c_void_p(start.data_ptr()), C.byref(n)))
         assert n.value == nc
         return cid, start, nc
+
+    def force_grid(self):
+        """{'ncell': (protons, neutrons), 'ncx': (protons, neutrons)} of the force path's per-species grids."""
+        out = (C.c_int32 * 4)()
+        _check(self.lib.pasta_force_grid(self._h, out))
+        return {"ncell": (out[0], out[2]), "ncx": (out[1], out[3])}
+
+    def force_cells(self):
+        """The force path's own cell list of the current positions: bin [N], bin_start [bins + 1], perm [N] (int32 cuda)."""
+        g = self.force_grid()
+        nbins = sum(nc * nc * ncx for nc, ncx in zip(g["ncell"], g["ncx"]))
+        i32 = self._torch.int32
+        b, start, perm = self._empty((self.N,), i32), self._empty((nbins + 1,), i32), self._empty((self.N,), i32)
+        _check(self.lib.pasta_force_cells(self._h, C.c_void_p(b.data_ptr()), C.c_void_p(start.data_ptr()),
+                                          C.c_void_p(perm.data_ptr())))
+        return b, start, perm, g
+
+    def list_stats(self):
+        out = (C.c_int64 * 2)()
+        _check(self.lib.pasta_list_stats(self._h, out))
+        return {"force_evals": int(out[0]), "list_builds": int(out[1])}
 
     def energy(self):
         ke, pe = C.c_double(), C.c_double()

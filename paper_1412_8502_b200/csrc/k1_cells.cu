@@ -258,7 +258,9 @@ __global__ void k1_chunk_rows_kernel(int32_t N, int32_t Np, const int32_t* __res
   // first slot of the row that slot `lo` belongs to
   const int sp0 = lo < Np ? 0 : 1;
   int row_lo = __ldg(bin_start + g.base[sp0] + (PASTA_CZ(c[0]) * g.ncell[sp0] + PASTA_CY(c[0])) * g.ncx[sp0]);
-  int first_slot[CHUNK_T], count[CHUNK_T];
+  // up to 2 * CHUNK_T - 1 pieces: a chunk can start at each of the 8 slots (row changes), and the nominal chunk
+  // that starts at the last one can be cut at the extent limit into up to 8 more
+  int first_slot[2 * CHUNK_T], count[2 * CHUNK_T];
   int m = 0;
 #pragma unroll
   for (int k = 0; k < CHUNK_T; ++k) {
@@ -354,18 +356,17 @@ static int auto_xsub(double L, double r_c, int k, int64_t n_species) {
   return xsub;
 }
 
-// Grids of the two species for the current box, buffers, and a zeroed histogram.  (The scatter kernel counts the
-// histogram back down to zero, so the memset is needed only when the table grows or somebody else used it.)
-int k1_setup(Sim* s, bool uniform_grid, GridPair* gp) {
+// Grids of the two species for the current box (host arithmetic only).
+void k1_grids(Sim* s, bool uniform_grid, GridPair* gp) {
   const int64_t N = s->N;
   // the reference kernel and the pair counter walk ONE isotropic grid; the chunk kernel takes a grid per
   // species, each cell sliced into thin cells along x (rows sorted in x: tight source ranges, compact chunks)
-  const bool uniform = uniform_grid || s->prm.force_variant == 1;
-  const bool same_k = uniform || s->prm.auto_grid == 0;
+  const bool uniform = uniform_grid || s->tune.force_variant == 1;
+  const bool same_k = uniform || s->tune.auto_grid == 0;
   const int k0 = same_k ? s->prm.cell_subdiv : auto_subdiv(s->L, s->prm.r_c, s->Np, s->prm.cell_subdiv);
   const int k1 = same_k ? s->prm.cell_subdiv : auto_subdiv(s->L, s->prm.r_c, N - s->Np, s->prm.cell_subdiv);
-  const int xs0 = uniform ? 1 : (s->prm.x_subdiv > 0 ? s->prm.x_subdiv : auto_xsub(s->L, s->prm.r_c, k0, s->Np));
-  const int xs1 = uniform ? 1 : (s->prm.x_subdiv > 0 ? s->prm.x_subdiv : auto_xsub(s->L, s->prm.r_c, k1, N - s->Np));
+  const int xs0 = uniform ? 1 : (s->tune.x_subdiv > 0 ? s->tune.x_subdiv : auto_xsub(s->L, s->prm.r_c, k0, s->Np));
+  const int xs1 = uniform ? 1 : (s->tune.x_subdiv > 0 ? s->tune.x_subdiv : auto_xsub(s->L, s->prm.r_c, k1, N - s->Np));
   s->grid_sp[0] = make_grid(s->L, s->prm.r_c, k0, xs0);
   s->grid_sp[1] = make_grid(s->L, s->prm.r_c, k1, xs1);
   GridPair& g = *gp;
@@ -381,6 +382,13 @@ int k1_setup(Sim* s, bool uniform_grid, GridPair* gp) {
   g.base[1] = (int)s->grid_sp[0].nc3;
   s->bin_base[0] = 0;
   s->bin_base[1] = s->grid_sp[0].nc3;
+}
+
+// The grids, the buffers, and a zeroed histogram.  (The scatter kernel counts the histogram back down to zero, so the
+// memset is needed only when the table grows or somebody else used it.)
+int k1_setup(Sim* s, bool uniform_grid, GridPair* gp) {
+  const int64_t N = s->N;
+  k1_grids(s, uniform_grid, gp);
   const int64_t nbins = s->grid_sp[0].nc3 + s->grid_sp[1].nc3;
   const void* before = s->bin_count.ptr;
   PASTA_TRY(buffer_reserve(s, &s->bin_count, sizeof(int32_t) * (size_t)(nbins + 1)));
@@ -396,7 +404,7 @@ int k1_setup(Sim* s, bool uniform_grid, GridPair* gp) {
 
 int k1_build(Sim* s, bool uniform_grid) {
   const int64_t N = s->N;
-  const bool uniform = uniform_grid || s->prm.force_variant == 1;
+  const bool uniform = uniform_grid || s->tune.force_variant == 1;
   GridPair g;
   const int B = 256;
   if (!(s->hist_valid && s->hist_uniform == uniform)) {

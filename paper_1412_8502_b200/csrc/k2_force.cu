@@ -213,7 +213,7 @@ static V0Args make_v0_args(Sim* s) {
 
 int k2_forces(Sim* s, bool with_energy) {
   // force_variant: 0 = library default (chunk kernel), 1 = thread-per-target reference, 2 = chunk kernel
-  if (s->prm.force_variant == 1) return k2_reference_forces(s, with_energy);
+  if (s->tune.force_variant == 1) return k2_reference_forces(s, with_energy);
   return k2_chunk_forces(s, with_energy, false);
 }
 

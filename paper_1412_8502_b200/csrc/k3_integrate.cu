@@ -120,7 +120,7 @@ int k3_kick_drift_count(Sim* s, double dt, double scale, double L_wrap) {
       dt, scale, L_wrap, 1.0 / L_wrap, g, s->cell_id.as<int32_t>(), s->bin_count.as<int32_t>());
   s->launches += 1;
   s->hist_valid = true;
-  s->hist_uniform = s->prm.force_variant == 1;
+  s->hist_uniform = s->tune.force_variant == 1;
   PASTA_CUDA_OK(cudaGetLastError());
   return PASTA_OK;
 }

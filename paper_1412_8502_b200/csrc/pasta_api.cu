@@ -4,6 +4,7 @@
 #include <math.h>
 #include <stdarg.h>
 #include <stdio.h>
+#include <stdlib.h>
 #include <string.h>
 
 #include <new>
@@ -110,7 +111,9 @@ static int evaluate_forces(Sim* s, bool with_energy) {
   {
     Timer t(s, 0);
     PASTA_TRY(k1_build(s));
+    s->n_list_builds += 1;
   }
+  s->n_force_evals += 1;
   {
     Timer t(s, 1);
     PASTA_TRY(k2_forces(s, with_energy));
@@ -148,11 +151,10 @@ int pasta_params_default(pasta_params* p) {
   p->scale_per_step = 1.0;
   p->thermostat_interval = 0;
   p->cell_subdiv = 4;
-  p->force_variant = 0;
   p->energy_every_step = 1;
-  p->auto_grid = 1;
-  p->x_subdiv = 0;
   p->skip_exact_zeros = 1;
+  p->list_reuse = 1;
+  p->list_halo = 0.0;
   p->r_nuc = 0.0;
   p->xi_dot = 0.0;
   return PASTA_OK;
@@ -164,9 +166,9 @@ static int validate_params(const pasta_params* p, double L) {
     return PASTA_EINVAL;
   }
   if (!(p->r_c > 0) || !(p->Lambda > 0) || !(p->lambda > 0) || !(p->mass > 0) || !(p->scale_per_step > 0) ||
-      p->thermostat_interval < 0 || p->cell_subdiv < 1 || p->cell_subdiv > 64 || p->force_variant < 0) {
+      p->thermostat_interval < 0 || p->cell_subdiv < 1 || p->cell_subdiv > 64 || !(p->list_halo >= 0.0)) {
     set_error("pasta_params: r_c, Lambda, lambda, mass, scale_per_step must be > 0, thermostat_interval >= 0, "
-              "1 <= cell_subdiv <= 64");
+              "1 <= cell_subdiv <= 64, list_halo >= 0");
     return PASTA_EINVAL;
   }
   if (!(p->r_nuc >= 0.0) || p->r_nuc > p->r_c) {
@@ -191,8 +193,8 @@ int pasta_create(pasta_sim** out, int64_t N, double Y_P, double density, double 
     return PASTA_EINVAL;
   }
   *out = nullptr;
-  if (N <= 0 || N > (1ll << 30) || !(Y_P >= 0.0 && Y_P <= 1.0) || !(density > 0.0) || !(T >= 0.0)) {
-    set_error("pasta_create: need 0 < N <= 2^30, 0 <= Y_P <= 1, density > 0, T >= 0");
+  if (N <= 0 || N >= (1ll << 26) || !(Y_P >= 0.0 && Y_P <= 1.0) || !(density > 0.0) || !(T >= 0.0)) {
+    set_error("pasta_create: need 0 < N < 2^26, 0 <= Y_P <= 1, density > 0, T >= 0");
     return PASTA_EINVAL;
   }
   const double L = cbrt((double)N / density);
@@ -207,6 +209,15 @@ int pasta_create(pasta_sim** out, int64_t N, double Y_P, double density, double 
     return PASTA_ENOMEM;
   }
   s->prm = *p;
+  {
+    auto env_int = [](const char* name, int dflt) {
+      const char* v = getenv(name);
+      return v && *v ? atoi(v) : dflt;
+    };
+    s->tune.force_variant = env_int("PASTA_FORCE_VARIANT", 0);
+    s->tune.auto_grid = env_int("PASTA_AUTO_GRID", 1);
+    s->tune.x_subdiv = env_int("PASTA_X_SUBDIV", 0);
+  }
   if (env) {
     s->env = *env;
   } else {
@@ -488,6 +499,53 @@ int pasta_cells(pasta_sim* sim, int32_t* cell_id_dev, int32_t* cell_start_dev, i
   return PASTA_OK;
 }
 
+int pasta_force_grid(pasta_sim* sim, int32_t* out4_host) {
+  Sim* s = reinterpret_cast<Sim*>(sim);
+  PASTA_TRY(check_sim(s));
+  if (!out4_host) {
+    set_error("out4_host is NULL");
+    return PASTA_EINVAL;
+  }
+  GridPair g;
+  k1_grids(s, false, &g);
+  for (int sp = 0; sp < 2; ++sp) {
+    out4_host[2 * sp + 0] = g.ncell[sp];
+    out4_host[2 * sp + 1] = g.ncx[sp];
+  }
+  return PASTA_OK;
+}
+
+int pasta_force_cells(pasta_sim* sim, int32_t* bin_dev, int32_t* bin_start_dev, int32_t* perm_dev) {
+  Sim* s = reinterpret_cast<Sim*>(sim);
+  PASTA_TRY(check_sim(s));
+  PASTA_TRY(use_device(s));
+  if (s->tune.force_variant == 1) {
+    set_error("pasta_force_cells: PASTA_FORCE_VARIANT=1 runs on the one isotropic grid that pasta_cells reports");
+    return PASTA_EINVAL;
+  }
+  // the list of the CURRENT positions, built by exactly the kernels a force evaluation runs
+  PASTA_TRY(k1_build(s));
+  const size_t n = (size_t)s->N;
+  const size_t nbins = (size_t)(s->grid_sp[0].nc3 + s->grid_sp[1].nc3);
+  if (bin_dev) PASTA_CUDA_OK(cudaMemcpyAsync(bin_dev, s->cell_id.ptr, 4 * n, cudaMemcpyDeviceToDevice, s->stream));
+  if (bin_start_dev)
+    PASTA_CUDA_OK(cudaMemcpyAsync(bin_start_dev, s->bin_start.ptr, 4 * (nbins + 1), cudaMemcpyDeviceToDevice, s->stream));
+  if (perm_dev) PASTA_CUDA_OK(cudaMemcpyAsync(perm_dev, s->perm.ptr, 4 * n, cudaMemcpyDeviceToDevice, s->stream));
+  return PASTA_OK;
+}
+
+int pasta_list_stats(pasta_sim* sim, int64_t* out2_host) {
+  Sim* s = reinterpret_cast<Sim*>(sim);
+  PASTA_TRY(check_sim(s));
+  if (!out2_host) {
+    set_error("out2_host is NULL");
+    return PASTA_EINVAL;
+  }
+  out2_host[0] = s->n_force_evals;
+  out2_host[1] = s->n_list_builds;
+  return PASTA_OK;
+}
+
 int pasta_energy(pasta_sim* sim, double* ke_host, double* pe_host) {
   Sim* s = reinterpret_cast<Sim*>(sim);
   PASTA_TRY(check_sim(s));
@@ -545,6 +603,10 @@ int pasta_force_stats(pasta_sim* sim, int64_t* out3_host) {
   PASTA_TRY(check_sim(s));
   if (!out3_host) {
     set_error("out3_host is NULL");
+    return PASTA_EINVAL;
+  }
+  if (s->tune.force_variant == 1) {
+    set_error("pasta_force_stats: only the chunk pair kernel keeps these statistics (PASTA_FORCE_VARIANT=1 is set)");
     return PASTA_EINVAL;
   }
   PASTA_TRY(use_device(s));

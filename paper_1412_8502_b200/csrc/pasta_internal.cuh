@@ -99,9 +99,18 @@ struct PairConsts {
 };
 PairConsts make_pair_consts(const pasta_params& p);
 
+// Tuning knobs that are not part of the ABI: read once per pasta_create from the environment
+// (PASTA_FORCE_VARIANT, PASTA_AUTO_GRID, PASTA_X_SUBDIV); the tests use them to cross-check kernels.
+struct Tuning {
+  int force_variant = 0;  // 0 = chunk kernel (production); 1 = thread-per-target kernel on one isotropic grid (k2_force.cu)
+  int auto_grid = 1;      // 1: each species' force grid picks its own k (about 8 particles per cell); 0: both use cell_subdiv
+  int x_subdiv = 0;       // thin cells along x per force-grid cell (0 = automatic: 8, fewer for a sparse species)
+};
+
 struct Sim {
   // configuration
   pasta_params prm;
+  Tuning tune;
   pasta_env env;
   cudaStream_t stream = nullptr;
   int64_t N = 0;
@@ -118,6 +127,8 @@ struct Sim {
   bool hist_uniform = false;  // ... built for the uniform (one grid) variant
   int64_t bins_zeroed = 0;    // bin_count[0, bins_zeroed) is known to be all zero (the scatter leaves it so)
   int64_t launches = 0;
+  int64_t n_force_evals = 0;  // force evaluations so far, and how many of them (re)built the cell list
+  int64_t n_list_builds = 0;
 
   // state (device)
   Buffer x, v, F, e, is_p;  // double[N][3] x3, double[N], uint8[N]
@@ -162,6 +173,7 @@ struct Sim {
 
 // ---- kernel launchers (one translation unit each) ---------------------------------------------------
 // K1  k1_cells.cu
+void k1_grids(Sim* s, bool uniform_grid, GridPair* g);  // the species' grids for the current L (host arithmetic only)
 int k1_setup(Sim* s, bool uniform_grid, GridPair* g);  // grids for the current L, buffers, a zeroed histogram
 int k1_build(Sim* s, bool uniform_grid = false);       // (species,cell) counting sort, pos4/perm, chunk table; uses the
                                                        // histogram of k3_kick_drift_count if s->hist_valid
