@@ -382,6 +382,7 @@ def run_sweep(args):
         pts.append({"step": done, "L_fm": L, "density": c["N"] / L ** 3, "steps_per_s": 1e3 * n / a.elapsed_time(b),
                     "PE_per_nucleon": pe / c["N"], "T_kin": ke / (1.5 * c["N"])})
     wall = time.perf_counter() - t_all0
+    list_stats = sim.list_stats()
     t0 = time.perf_counter()
     label, ncl = sim.clusters(c["r_cl"])
     A, Z = sim.cluster_sizes()
@@ -400,7 +401,7 @@ def run_sweep(args):
     for a_, z_ in zip(A[heavy].tolist(), Z[heavy].tolist()):
         hist[(a_ // 20 * 20, z_ // 10 * 10)] = hist.get((a_ // 20 * 20, z_ // 10 * 10), 0) + 1
     line = {"sweep": args.sweep, "workload": workload_config(args.sweep, 1)["workload"] + ", decompression to 0.00125 fm^-3",
-            "steps": c["steps"], "wall_s": wall, "points": pts, "clusters": ncl, "fof_s": fof_s, "composition": comp,
+            "steps": c["steps"], "wall_s": wall, "list_stats": list_stats, "points": pts, "clusters": ncl, "fof_s": fof_s, "composition": comp,
             "mst_r_pp_4.5_r_np_3.0": {"clusters": ncl_mst, "composition": comp_mst}, "largest_A": int(A.max()), "AZ_histogram_A20_Z10_bins": {"%d,%d" % k: v for k, v in sorted(hist.items())}}
     print(json.dumps(line), flush=True)
     sim.close()

@@ -64,7 +64,7 @@ typedef struct pasta_params {
                                   source-segment list are built with a halo (skin) and kept across steps until some particle
                                   has moved more than half the halo -- the paper's neighbour list with its displacement
                                   trigger.  F and e do not depend on it.  0: rebuild every step */
-  double list_halo;            /* halo thickness delta_r in fm (4 fm); 0 = library default */
+  double list_halo;            /* halo thickness delta_r in fm (PAPER.md:126 uses 4 fm); 0 = library default (6 fm) */
   double r_nuc;                /* > 0: the paper's own range split: the nuclear (Gaussian) terms are zero
                                   and not computed beyond r_nuc (11.5 fm in the paper) while the Coulomb term still reaches
                                   r_c.  0 (default): one cut-off r_c for every term (D1).  Must be <= r_c */

@@ -12,6 +12,10 @@
 //   cxyz[N]               cx | cy << 12 | cz << 22
 // pasta_cells() exports the species-independent O3 grid of pasta_params.cell_subdiv with the same
 // cell_coord arithmetic.
+#include <string.h>
+
+#include <chrono>
+
 #include "pasta_internal.cuh"
 
 namespace pasta {
@@ -171,12 +175,13 @@ __global__ void k1_order_kernel(int64_t nbins, const int32_t* __restrict__ bin_s
 // (and with it the summation order of the force kernel) is ascending in the original index whatever the
 // arrival order was, and writes it to `perm_out`.  (Thin-cell bins hold a particle or two; the uniform one-grid
 // variant, whose bins hold hundreds, orders them with k1_order_kernel instead.)
+// list_format (k2_list.cu): pos4.w carries the bits of the packed cell coordinates instead of the thin-cell index as a float.
 template <bool FUSED_ORDER>
 __global__ void k1_gather_kernel(int64_t N, const double* __restrict__ x, const int32_t* __restrict__ pbin,
                                  const int32_t* __restrict__ perm_in, int32_t* __restrict__ perm_out,
                                  const int32_t* __restrict__ bin_start, const GridPair g, double sigma,
                                  float4* __restrict__ pos4, int32_t* __restrict__ cxyz,
-                                 int32_t* __restrict__ zero_me) {
+                                 int32_t* __restrict__ zero_me, bool list_format, int32_t* __restrict__ slot_of) {
   int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (t == 0 && zero_me) *zero_me = 0;  // the overflow counter of the chunk table
   if (t >= N) return;
@@ -195,6 +200,7 @@ __global__ void k1_gather_kernel(int64_t N, const double* __restrict__ x, const 
     }
     perm_out[t] = i;
   }
+  if (slot_of) slot_of[i] = (int32_t)t;
   const int sp = bin >= g.base[1] ? 1 : 0;
   const int id = bin - g.base[sp], nc = g.ncell[sp], ncx = g.ncx[sp];
   const double w = g.w[sp];
@@ -203,9 +209,10 @@ __global__ void k1_gather_kernel(int64_t N, const double* __restrict__ x, const 
   p.x = (float)(sigma * (x[3 * i + 0] - ((double)cx + 0.5) * g.wx[sp]));
   p.y = (float)(sigma * (x[3 * i + 1] - ((double)cy + 0.5) * w));
   p.z = (float)(sigma * (x[3 * i + 2] - ((double)cz + 0.5) * w));
-  p.w = (float)cx;
+  const int packed = cx | (cy << 12) | (cz << 22);
+  p.w = list_format ? __int_as_float(packed) : (float)cx;
   pos4[t] = p;
-  cxyz[t] = cx | (cy << 12) | (cz << 22);
+  cxyz[t] = packed;
 }
 
 // Chunk table of the pair kernel.  A chunk = the targets of one warp = up to CHUNK_T sorted slots of one species
@@ -356,39 +363,80 @@ static int auto_xsub(double L, double r_c, int k, int64_t n_species) {
   return xsub;
 }
 
+// ---- list mode (k2_list.cu) -------------------------------------------------------------------------------------------
+// One grid for both species, cells as wide as the precision cap allows, no thin cells: rows are only listed when the
+// lists are built.
+static int list_subdiv(const Sim* s) { return (int)ceil(s->prm.r_c / PASTA_WMAX); }
+
+// The paper's delta_r is 4 fm for a CPU list; here a rebuild costs ten force evaluations and a list entry
+// little, and 6 fm measured best at the dilute ends of configs 3 and 5 (profiles/).
+double list_halo(const Sim* s) { return s->prm.list_halo > 0.0 ? s->prm.list_halo : 6.0; }
+
+// Lists pay where both species are sparse on that grid (fewer than 3 per cell: the regime of the SPARSE chunk
+// builder), i.e. the cold dilute end of a decompression (rebuilt every ~100 steps there); and the box
+// must be wide enough for cell offsets to have one nearest image within reach + halo of a chunk.
+bool list_mode_wanted(const Sim* s) {
+  if (!s->prm.list_reuse || s->tune.force_variant != 0 || s->no_lists) return false;
+  if (s->L < 2.0 * (s->prm.r_c + list_halo(s)) + 6.0 * PASTA_WMAX) return false;
+  if (s->N > (1 << 20)) return false;  // a list entry packs the sorted slot in 20 bits ...
+  const Grid g = make_grid(s->L, s->prm.r_c, list_subdiv(s), 1);
+  if (g.ncell < 4) return false;
+  if (ceil((s->prm.r_c + list_halo(s)) / g.w + 1e-3) > 7.0) return false;  // ... and a cell offset in 4 signed bits
+  const double n_max = (double)(s->Np > s->N - s->Np ? s->Np : s->N - s->Np);
+  return n_max / ((double)g.ncell * g.ncell * g.ncell) < 3.0;
+}
+
+static void fill_grid_pair(const Grid gr[2], GridPair* gp) {
+  GridPair& g = *gp;
+  for (int sp = 0; sp < 2; ++sp) {
+    g.ncell[sp] = gr[sp].ncell;
+    g.ncx[sp] = gr[sp].ncx;
+    g.inv_w[sp] = gr[sp].inv_w;
+    g.w[sp] = gr[sp].w;
+    g.inv_wx[sp] = gr[sp].inv_wx;
+    g.wx[sp] = gr[sp].wx;
+  }
+  g.base[0] = 0;
+  g.base[1] = (int)gr[0].nc3;
+}
+
+// The frozen cell counts of s->grid_sp with the widths of the current box side (the grid scales with the box).
+void k1_frozen_grids(Sim* s, GridPair* gp) {
+  for (int sp = 0; sp < 2; ++sp) {
+    Grid& g = s->grid_sp[sp];
+    g.inv_w = (double)g.ncell / s->L;
+    g.w = s->L / (double)g.ncell;
+    g.inv_wx = (double)g.ncx / s->L;
+    g.wx = s->L / (double)g.ncx;
+  }
+  fill_grid_pair(s->grid_sp, gp);
+}
+
 // Grids of the two species for the current box (host arithmetic only).
-void k1_grids(Sim* s, bool uniform_grid, GridPair* gp) {
+void k1_grids(const Sim* s, bool uniform_grid, Grid out[2], GridPair* gp) {
   const int64_t N = s->N;
   // the reference kernel and the pair counter walk ONE isotropic grid; the chunk kernel takes a grid per
   // species, each cell sliced into thin cells along x (rows sorted in x: tight source ranges, compact chunks)
   const bool uniform = uniform_grid || s->tune.force_variant == 1;
+  const bool lists = !uniform && list_mode_wanted(s);
   const bool same_k = uniform || s->tune.auto_grid == 0;
-  const int k0 = same_k ? s->prm.cell_subdiv : auto_subdiv(s->L, s->prm.r_c, s->Np, s->prm.cell_subdiv);
-  const int k1 = same_k ? s->prm.cell_subdiv : auto_subdiv(s->L, s->prm.r_c, N - s->Np, s->prm.cell_subdiv);
-  const int xs0 = uniform ? 1 : (s->tune.x_subdiv > 0 ? s->tune.x_subdiv : auto_xsub(s->L, s->prm.r_c, k0, s->Np));
-  const int xs1 = uniform ? 1 : (s->tune.x_subdiv > 0 ? s->tune.x_subdiv : auto_xsub(s->L, s->prm.r_c, k1, N - s->Np));
-  s->grid_sp[0] = make_grid(s->L, s->prm.r_c, k0, xs0);
-  s->grid_sp[1] = make_grid(s->L, s->prm.r_c, k1, xs1);
-  GridPair& g = *gp;
-  for (int sp = 0; sp < 2; ++sp) {
-    g.ncell[sp] = s->grid_sp[sp].ncell;
-    g.ncx[sp] = s->grid_sp[sp].ncx;
-    g.inv_w[sp] = s->grid_sp[sp].inv_w;
-    g.w[sp] = s->grid_sp[sp].w;
-    g.inv_wx[sp] = s->grid_sp[sp].inv_wx;
-    g.wx[sp] = s->grid_sp[sp].wx;
-  }
-  g.base[0] = 0;
-  g.base[1] = (int)s->grid_sp[0].nc3;
-  s->bin_base[0] = 0;
-  s->bin_base[1] = s->grid_sp[0].nc3;
+  const int k0 = lists ? list_subdiv(s) : same_k ? s->prm.cell_subdiv : auto_subdiv(s->L, s->prm.r_c, s->Np, s->prm.cell_subdiv);
+  const int k1 = lists ? list_subdiv(s) : same_k ? s->prm.cell_subdiv : auto_subdiv(s->L, s->prm.r_c, N - s->Np, s->prm.cell_subdiv);
+  const int xs0 = uniform || lists ? 1 : (s->tune.x_subdiv > 0 ? s->tune.x_subdiv : auto_xsub(s->L, s->prm.r_c, k0, s->Np));
+  const int xs1 = uniform || lists ? 1 : (s->tune.x_subdiv > 0 ? s->tune.x_subdiv : auto_xsub(s->L, s->prm.r_c, k1, N - s->Np));
+  out[0] = make_grid(s->L, s->prm.r_c, k0, xs0);
+  out[1] = make_grid(s->L, s->prm.r_c, k1, xs1);
+  fill_grid_pair(out, gp);
 }
 
 // The grids, the buffers, and a zeroed histogram.  (The scatter kernel counts the histogram back down to zero, so the
 // memset is needed only when the table grows or somebody else used it.)
 int k1_setup(Sim* s, bool uniform_grid, GridPair* gp) {
   const int64_t N = s->N;
-  k1_grids(s, uniform_grid, gp);
+  s->list.valid = false;  // whoever sets the grids up again is about to re-sort
+  k1_grids(s, uniform_grid, s->grid_sp, gp);
+  s->bin_base[0] = 0;
+  s->bin_base[1] = s->grid_sp[0].nc3;
   const int64_t nbins = s->grid_sp[0].nc3 + s->grid_sp[1].nc3;
   const void* before = s->bin_count.ptr;
   PASTA_TRY(buffer_reserve(s, &s->bin_count, sizeof(int32_t) * (size_t)(nbins + 1)));
@@ -405,6 +453,7 @@ int k1_setup(Sim* s, bool uniform_grid, GridPair* gp) {
 int k1_build(Sim* s, bool uniform_grid) {
   const int64_t N = s->N;
   const bool uniform = uniform_grid || s->tune.force_variant == 1;
+  const bool lists = !uniform && list_mode_wanted(s);  // per-target neighbour lists follow: no chunk table
   GridPair g;
   const int B = 256;
   if (!(s->hist_valid && s->hist_uniform == uniform)) {
@@ -428,18 +477,19 @@ int k1_build(Sim* s, bool uniform_grid) {
     k1_order_kernel<<<grid_for(nbins, B), B, 0, s->stream>>>(nbins, start, s->perm.as<int32_t>());
     k1_gather_kernel<false><<<grid_for(N, B), B, 0, s->stream>>>(N, s->x.as<double>(), s->cell_id.as<int32_t>(),
                                                                  s->perm.as<int32_t>(), nullptr, start, g, sigma,
-                                                                 s->pos4.as<float4>(), s->cxyz.as<int32_t>(), nullptr);
+                                                                 s->pos4.as<float4>(), s->cxyz.as<int32_t>(), nullptr, false, nullptr);
     s->launches += 3;
   } else {
+    if (lists) PASTA_TRY(buffer_reserve(s, &s->slot_of, sizeof(int32_t) * (size_t)N));
     k1_scatter_kernel<<<grid_for(N, B), B, 0, s->stream>>>(N, s->cell_id.as<int32_t>(), start, cnt,
                                                            s->perm_raw.as<int32_t>());
     k1_gather_kernel<true><<<grid_for(N, B), B, 0, s->stream>>>(N, s->x.as<double>(), s->cell_id.as<int32_t>(),
                                                                 s->perm_raw.as<int32_t>(), s->perm.as<int32_t>(), start,
                                                                 g, sigma, s->pos4.as<float4>(), s->cxyz.as<int32_t>(),
-                                                                n_overflow);
+                                                                n_overflow, lists, lists ? s->slot_of.as<int32_t>() : nullptr);
     s->launches += 2;
   }
-  if (!uniform) {
+  if (!uniform && !lists) {
     // builder per species (DENSE row runs: at least 3 particles per cell on average), the extent limit of a row
     // run (three cell widths, at most 16 fm) and the capacity of the table: a bound on the number of chunks
     //   row runs: primary entries ceil(N / 8); overflow <= one per row (row or species change inside 8 slots)
@@ -491,6 +541,75 @@ int k1_build(Sim* s, bool uniform_grid) {
   }
   PASTA_CUDA_OK(cudaGetLastError());
   return PASTA_OK;
+}
+
+// ---- list mode: the frozen sorted order, refreshed ----------------------------------------------------------------------
+// Sorted slot t keeps its particle perm[t] and its cell cxyz[t] from the last build; the particle has moved (and the
+// grid has scaled with the box), so pos4[t] = sigma * (x - centre of that cell) in the nearest image -- the arithmetic
+// of k1_gather_kernel, which it reproduces bit for bit for a particle that is still inside its cell.  With it, the
+// trigger of the paper's neighbour list: the largest displacement since the build, measured in
+// co-moving coordinates u = x / L (a uniform scaling of the box moves nothing) and expressed at the build's box side.
+// The last block to finish posts {seq, max displacement^2} to the host's mailbox and re-arms the scratch words.
+__global__ void __launch_bounds__(256) k1_refresh_kernel(int32_t N, const double* __restrict__ x,
+                                                         const int32_t* __restrict__ perm, const RefreshArgs R) {
+  const int t = blockIdx.x * blockDim.x + threadIdx.x;
+  float d2 = 0.f;
+  if (t < N) {
+    const int64_t i = perm[t];
+    const double xi[3] = {x[3 * i + 0], x[3 * i + 1], x[3 * i + 2]};
+    d2 = refresh_slot(R, t, i, xi);
+  }
+  refresh_post(R, d2);
+}
+
+void k1_refresh_args(Sim* s, RefreshArgs* out) {
+  RefreshArgs& R = *out;
+  k1_frozen_grids(s, &R.g);
+  R.xref = s->xref.as<double>();
+  R.cxyz = s->cxyz.as<int32_t>();
+  R.pos4 = s->pos4.as<float4>();
+  R.Np = (int32_t)s->Np;
+  R.sigma = sqrt(1.4426950408889634074 / (2.0 * s->prm.Lambda));
+  R.L = s->L;
+  R.invL = 1.0 / s->L;
+  R.L0 = s->list.L0;
+  R.invL0 = 1.0 / s->list.L0;
+  R.scratch = s->counters.as<unsigned>() + 2 * 28;  // counters[28]: {max bits, ticket}
+  R.mbox = s->list.mbox_dev;
+  R.seq = ++s->list.seq;
+}
+
+// The host decides whether the lists survive this step: wait for the post of the refresh (a few microseconds after
+// the kernel ends).
+int k1_refresh_wait(Sim* s, double* max_disp_host) {
+  const unsigned seq = s->list.seq;
+  s->list.pending = false;
+  const auto t0 = std::chrono::steady_clock::now();
+  unsigned long long m;
+  int spins = 0;
+  while ((unsigned)((m = *s->list.mbox_host) >> 32) != seq) {
+    if ((++spins & 0xfff) == 0 && std::chrono::steady_clock::now() - t0 > std::chrono::seconds(20)) {
+      PASTA_CUDA_OK(cudaStreamSynchronize(s->stream));
+      if ((unsigned)((m = *s->list.mbox_host) >> 32) != seq) {
+        set_error("k1_refresh: the displacement readback never arrived");
+        return PASTA_ECUDA;
+      }
+    }
+  }
+  float f;
+  const unsigned bits = (unsigned)(m & 0xffffffffu);
+  memcpy(&f, &bits, sizeof(f));
+  *max_disp_host = sqrt((double)f);
+  return PASTA_OK;
+}
+
+int k1_refresh(Sim* s, double* max_disp_host) {
+  RefreshArgs R;
+  k1_refresh_args(s, &R);
+  k1_refresh_kernel<<<grid_for(s->N, 256), 256, 0, s->stream>>>((int32_t)s->N, s->x.as<double>(), s->perm.as<int32_t>(), R);
+  s->launches += 1;
+  PASTA_CUDA_OK(cudaGetLastError());
+  return k1_refresh_wait(s, max_disp_host);
 }
 
 // pasta_cells: the O3 grid of cell_subdiv, species-independent (uses the cell-list scratch buffers; the next

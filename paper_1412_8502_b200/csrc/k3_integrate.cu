@@ -1,6 +1,8 @@
 // K3 -- velocity Verlet, isokinetic rescale and uniform box/position scaling in FP64
 // (readings D6-D11), plus the seeded initial state (D15)
 // and the deterministic FP64 reductions (KE, PE).
+#include <string.h>
+
 #include "pasta_internal.cuh"
 
 namespace pasta {
@@ -31,9 +33,32 @@ __global__ void k3_kick_drift_count_kernel(int64_t N, double* __restrict__ x, do
     xn[k] = wrap_coord(scale * (x[3 * i + k] + dt * vk), L, invL);
     x[3 * i + k] = xn[k];
   }
+  if (bin_count == nullptr) return;  // list mode: the sorted order is frozen (or about to be rebuilt on another grid)
   const int bin = force_bin(g, is_p[i] ? 0 : 1, xn[0], xn[1], xn[2]);
   pbin[i] = bin;
   atomicAdd(&bin_count[bin], 1);
+}
+
+// List mode: the same kick and drift, and fused with it the refresh of the frozen sorted order (k1_refresh_kernel): the
+// particle's slot gets its new cell-relative coordinates and the launch reports the largest displacement since the build.
+__global__ void __launch_bounds__(128) k3_kick_drift_refresh_kernel(int64_t N, double* __restrict__ x, double* __restrict__ v,
+                                                                    const double* __restrict__ F, double h, double dt,
+                                                                    double scale, double L, double invL,
+                                                                    const int32_t* __restrict__ slot_of, const RefreshArgs R) {
+  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  float d2 = 0.f;
+  if (i < N) {
+    double xn[3];
+#pragma unroll
+    for (int k = 0; k < 3; ++k) {
+      const double vk = v[3 * i + k] + h * F[3 * i + k];
+      v[3 * i + k] = vk;
+      xn[k] = wrap_coord(scale * (x[3 * i + k] + dt * vk), L, invL);
+      x[3 * i + k] = xn[k];
+    }
+    d2 = refresh_slot(R, slot_of[i], i, xn);
+  }
+  refresh_post(R, d2);
 }
 
 constexpr int RED_T = 256;
@@ -112,15 +137,29 @@ static int red_blocks(int64_t n) {
 
 // The caller has set s->L to the box the forces will be evaluated in; L_wrap = the box the drifted positions are
 // wrapped into (the same, except under the linear box-only expansion, where it is the box before it grew).
-int k3_kick_drift_count(Sim* s, double dt, double scale, double L_wrap) {
+int k3_kick_drift_count(Sim* s, double dt, double scale, double L_wrap, bool count) {
   GridPair g;
-  PASTA_TRY(k1_setup(s, false, &g));
+  memset(&g, 0, sizeof(g));
+  if (count) PASTA_TRY(k1_setup(s, false, &g));
   k3_kick_drift_count_kernel<<<grid_for(s->N, 128), 128, 0, s->stream>>>(
       s->N, s->x.as<double>(), s->v.as<double>(), s->F.as<double>(), s->is_p.as<uint8_t>(), dt / (2.0 * s->prm.mass),
-      dt, scale, L_wrap, 1.0 / L_wrap, g, s->cell_id.as<int32_t>(), s->bin_count.as<int32_t>());
+      dt, scale, L_wrap, 1.0 / L_wrap, g, s->cell_id.as<int32_t>(), count ? s->bin_count.as<int32_t>() : nullptr);
   s->launches += 1;
-  s->hist_valid = true;
+  s->hist_valid = count;
   s->hist_uniform = s->tune.force_variant == 1;
+  PASTA_CUDA_OK(cudaGetLastError());
+  return PASTA_OK;
+}
+
+int k3_kick_drift_refresh(Sim* s, double dt, double scale, double L_wrap) {
+  RefreshArgs R;
+  k1_refresh_args(s, &R);
+  k3_kick_drift_refresh_kernel<<<grid_for(s->N, 128), 128, 0, s->stream>>>(
+      s->N, s->x.as<double>(), s->v.as<double>(), s->F.as<double>(), dt / (2.0 * s->prm.mass), dt, scale, L_wrap,
+      1.0 / L_wrap, s->slot_of.as<int32_t>(), R);
+  s->launches += 1;
+  s->hist_valid = false;
+  s->list.pending = true;
   PASTA_CUDA_OK(cudaGetLastError());
   return PASTA_OK;
 }

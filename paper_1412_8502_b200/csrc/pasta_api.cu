@@ -57,7 +57,8 @@ void buffer_release(Sim* s, Buffer* b) {
 static void release_all(Sim* s) {
   Buffer* bs[] = {&s->x, &s->v, &s->F, &s->e, &s->is_p, &s->cell_id, &s->bin_count, &s->bin_start, &s->scan_tmp,
                   &s->perm, &s->perm_raw, &s->pos4, &s->cxyz, &s->partials, &s->scalars, &s->counters, &s->cl_parent, &s->cl_A,
-                  &s->cl_Z, &s->cl_cell_id, &s->cl_count, &s->cl_start, &s->cl_perm, &s->chunk_tab};
+                  &s->cl_Z, &s->cl_cell_id, &s->cl_count, &s->cl_start, &s->cl_perm, &s->chunk_tab, &s->xref, &s->slot_of, &s->list_off,
+                  &s->list_pool};
   for (Buffer* b : bs) buffer_release(s, b);
 }
 
@@ -107,21 +108,58 @@ struct Timer {
   }
 };
 
-static int evaluate_forces(Sim* s, bool with_energy) {
-  {
-    Timer t(s, 0);
-    PASTA_TRY(k1_build(s));
-    s->n_list_builds += 1;
-  }
+// One force evaluation of the current positions.  Dense regime: sort + chunk table (K1), chunk kernel (K2).  Where
+// list_mode_wanted(): the paper's neighbour list -- sort, chunk table and per-chunk source lists are
+// built with a halo and reused; every evaluation first refreshes the sorted coordinates and reads back the largest
+// displacement D since the build, and rebuilds when a pair could have entered the reach unseen:
+//   own + source displacement 2 D > halo  (less reach (L0/L - 1) if the box has shrunk since).
+static int evaluate_forces_tail(Sim* s, bool with_energy) {
   s->n_force_evals += 1;
   {
     Timer t(s, 1);
-    PASTA_TRY(k2_forces(s, with_energy));
+    if (s->list.valid) PASTA_TRY(k2_list_forces(s, with_energy));
+    else PASTA_TRY(k2_forces(s, with_energy));
   }
   if (s->timing) s->n_timed += 1;
   s->forces_valid = true;
   s->energies_valid = with_energy;
   return PASTA_OK;
+}
+
+static int evaluate_forces(Sim* s, bool with_energy) {
+  {
+    Timer t(s, 0);
+    if (s->list.valid) {
+      double d = 0.0;
+      if (s->list.pending) PASTA_TRY(k1_refresh_wait(s, &d));  // the kick-drift kernel of this step carried the refresh
+      else PASTA_TRY(k1_refresh(s, &d));
+      const double ratio = s->L / s->list.L0;
+      const double delta = s->list.halo + (ratio >= 1.0 ? 0.0 : s->prm.r_c * (1.0 - 1.0 / ratio));
+      // (the frozen grid scales with the box: 5 % keeps the cells within the width the FP32 coordinates are good for)
+      if (!(2.0 * d <= delta) || ratio > 1.05 || ratio < 0.95 || !list_mode_wanted(s)) s->list.valid = false;
+    }
+    if (!s->list.valid) {
+      const bool lists = list_mode_wanted(s);
+      PASTA_TRY(k1_build(s));
+      s->n_list_builds += 1;
+      if (lists) {
+        const double halo = list_halo(s);
+        const int rc = k2_list_build(s, halo);
+        if (rc == 1) {  // too dense for lists after all (a clustered state): the chunk kernel on its own sort, from now on
+          s->no_lists = true;
+          PASTA_TRY(k1_build(s));
+          return evaluate_forces_tail(s, with_energy);
+        }
+        PASTA_TRY(rc);
+        PASTA_TRY(buffer_reserve(s, &s->xref, 24 * (size_t)s->N));
+        PASTA_CUDA_OK(cudaMemcpyAsync(s->xref.ptr, s->x.ptr, 24 * (size_t)s->N, cudaMemcpyDeviceToDevice, s->stream));
+        s->list.L0 = s->L;
+        s->list.halo = halo;
+        s->list.valid = true;
+      }
+    }
+  }
+  return evaluate_forces_tail(s, with_energy);
 }
 
 }  // namespace pasta
@@ -249,7 +287,19 @@ int pasta_create(pasta_sim** out, int64_t N, double Y_P, double density, double 
         (rc = buffer_reserve(s, &s->cxyz, 4 * n)) || (rc = buffer_reserve(s, &s->partials, 8 * 8192)) ||
         (rc = buffer_reserve(s, &s->scalars, 8 * 16)) || (rc = buffer_reserve(s, &s->counters, 8 * 32)))
       break;
-    if (cudaMemsetAsync(s->F.ptr, 0, 24 * n, s->stream) != cudaSuccess ||
+    {
+      void* mb = nullptr;
+      if (cudaHostAlloc(&mb, 64, cudaHostAllocMapped) != cudaSuccess ||
+          cudaHostGetDevicePointer(reinterpret_cast<void**>(&s->list.mbox_dev), mb, 0) != cudaSuccess) {
+        set_error("pinned mailbox allocation failed: %s", cudaGetErrorString(cudaGetLastError()));
+        rc = PASTA_ECUDA;
+        break;
+      }
+      memset(mb, 0, 64);
+      s->list.mbox_host = reinterpret_cast<volatile unsigned long long*>(mb);
+    }
+    if (cudaMemsetAsync(s->counters.ptr, 0, 8 * 32, s->stream) != cudaSuccess ||
+        cudaMemsetAsync(s->F.ptr, 0, 24 * n, s->stream) != cudaSuccess ||
         cudaMemsetAsync(s->e.ptr, 0, 8 * n, s->stream) != cudaSuccess ||
         cudaMemsetAsync(s->scalars.ptr, 0, 8 * 16, s->stream) != cudaSuccess) {
       set_error("cudaMemsetAsync failed: %s", cudaGetErrorString(cudaGetLastError()));
@@ -272,6 +322,7 @@ int pasta_destroy(pasta_sim* sim) {
   cudaSetDevice(s->env.device);
   cudaStreamSynchronize(s->stream);
   release_all(s);
+  if (s->list.mbox_host) cudaFreeHost(const_cast<unsigned long long*>(s->list.mbox_host));
   for (cudaEvent_t e : s->evs)
     if (e) cudaEventDestroy(e);
   delete s;
@@ -316,7 +367,10 @@ int pasta_step(pasta_sim* sim, int64_t n, double dt) {
     s->L = L_new;
     {
       Timer t(s, 2);
-      PASTA_TRY(k3_kick_drift_count(s, dt, sc, linear ? L_old : L_new));
+      // the cell histogram of the new positions rides along unless the sorted order is frozen (or about to be
+      // rebuilt on the lists' own grid)
+      if (s->list.valid) PASTA_TRY(k3_kick_drift_refresh(s, dt, sc, linear ? L_old : L_new));
+      else PASTA_TRY(k3_kick_drift_count(s, dt, sc, linear ? L_old : L_new, !list_mode_wanted(s)));
       s->lin_n += 1;
     }
     s->clusters_valid = false;
@@ -341,6 +395,7 @@ int pasta_expand(pasta_sim* sim, double scale) {
   PASTA_TRY(use_device(s));
   const double L_new = s->L * scale;
   PASTA_TRY(k3_wrap_scale(s, scale, L_new));
+  s->list.valid = false;
   s->L = L_new;
   s->lin_L0 = L_new;
   s->lin_n = 0;
@@ -416,6 +471,7 @@ int pasta_get_state(pasta_sim* sim, double* x_dev, double* v_dev, uint8_t* is_pr
 }
 
 static int after_set_state(Sim* s, bool have_is_p, bool have_F, double L) {
+  s->list.valid = false;
   s->L = L;
   s->lin_L0 = L;
   s->lin_n = 0;
@@ -507,7 +563,8 @@ int pasta_force_grid(pasta_sim* sim, int32_t* out4_host) {
     return PASTA_EINVAL;
   }
   GridPair g;
-  k1_grids(s, false, &g);
+  Grid gr[2];
+  k1_grids(s, false, gr, &g);
   for (int sp = 0; sp < 2; ++sp) {
     out4_host[2 * sp + 0] = g.ncell[sp];
     out4_host[2 * sp + 1] = g.ncx[sp];
@@ -610,7 +667,11 @@ int pasta_force_stats(pasta_sim* sim, int64_t* out3_host) {
     return PASTA_EINVAL;
   }
   PASTA_TRY(use_device(s));
-  PASTA_TRY(k1_build(s));
+  const bool no_lists = s->no_lists;
+  s->no_lists = true;  // the statistics are the chunk kernel's: sort on its own grids even where lists would be used
+  int rc = k1_build(s);
+  s->no_lists = no_lists;
+  PASTA_TRY(rc);
   PASTA_TRY(k2_chunk_forces(s, true, true));
   s->forces_valid = true;
   s->energies_valid = true;

@@ -81,6 +81,64 @@ __device__ __forceinline__ int force_bin(const GridPair& g, int sp, double x, do
 }
 #endif
 
+#ifdef __CUDACC__
+// List mode (k2_list.cu): what the frozen sorted order needs of a moved particle (k1_refresh_kernel; fused into the
+// kick-drift kernel of a step).
+struct RefreshArgs {
+  const double* xref;     // positions at the list build
+  const int32_t* cxyz;    // [slot] frozen packed cell coordinates
+  float4* pos4;           // [slot] out
+  GridPair g;             // the frozen cell counts with the widths of the current box
+  int32_t Np;
+  double sigma, L, invL, L0, invL0;
+  unsigned* scratch;      // {max displacement^2 (float bits), blocks finished}; zero between launches
+  unsigned long long* mbox;
+  unsigned seq;
+};
+// pos4[slot] = sigma * (x - centre of the slot's frozen cell), nearest image -- bit for bit k1_gather_kernel's value
+// while the particle is inside its cell; returns its squared displacement since the build, measured in co-moving
+// coordinates u = x / L and expressed at the build's box side (the trigger of the neighbour list).
+__device__ __forceinline__ float refresh_slot(const RefreshArgs& R, const int slot, const int64_t i, const double* xi) {
+  const int c = R.cxyz[slot], sp = slot < R.Np ? 0 : 1;
+  const int cc[3] = {PASTA_CX(c), PASTA_CY(c), PASTA_CZ(c)};
+  const double wa[3] = {R.g.wx[sp], R.g.w[sp], R.g.w[sp]};
+  float p[3];
+  double dd2 = 0.0;
+#pragma unroll
+  for (int a = 0; a < 3; ++a) {
+    double d = xi[a] - ((double)cc[a] + 0.5) * wa[a];
+    d -= R.L * rint(d * R.invL);
+    p[a] = (float)(R.sigma * d);
+    double du = xi[a] * R.invL - R.xref[3 * i + a] * R.invL0;
+    du -= rint(du);
+    du *= R.L0;
+    dd2 += du * du;
+  }
+  R.pos4[slot] = make_float4(p[0], p[1], p[2], __int_as_float(c));
+  return __double2float_ru(dd2);
+}
+// Block maximum of d2, folded into the launch's maximum; the last block to finish posts {seq, maximum} to the host's
+// mailbox and re-arms the scratch words.  Every thread of the block must call it.  blockDim.x <= 256.
+__device__ __forceinline__ void refresh_post(const RefreshArgs& R, float d2) {
+  __shared__ float wmax[8];
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) d2 = fmaxf(d2, __shfl_xor_sync(0xffffffffu, d2, o));
+  if ((threadIdx.x & 31) == 0) wmax[threadIdx.x >> 5] = d2;
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    for (int k = 1; k < (int)(blockDim.x >> 5); ++k) d2 = fmaxf(d2, wmax[k]);
+    atomicMax(R.scratch, __float_as_uint(d2));  // d2 >= 0: the bit patterns order like the values
+    __threadfence();
+    if (atomicAdd(R.scratch + 1, 1u) == gridDim.x - 1) {
+      const unsigned m = atomicExch(R.scratch, 0u);
+      R.scratch[1] = 0u;
+      *reinterpret_cast<volatile unsigned long long*>(R.mbox) = ((unsigned long long)R.seq << 32) | m;
+      __threadfence_system();
+    }
+  }
+}
+#endif
+
 // Constants of the FP32 pair arithmetic, derived on the host in FP64 (k2_force.cu explains them).
 struct PairConsts {
   float sigma;       // coordinate pre-scale sqrt(log2(e) / (2 Lambda))
@@ -154,6 +212,23 @@ struct Sim {
   Buffer cl_parent, cl_A, cl_Z;  // int32[N] each
   Buffer cl_cell_id, cl_count, cl_start, cl_perm;
 
+  // reused neighbour lists (k2_list.cu).  While list.valid the sorted order (perm, cxyz), the cell
+  // counts of grid_sp, the chunk table and the lists are FROZEN; pos4 is refreshed from x every step.
+  struct ListState {
+    bool valid = false;     // the frozen order and the lists describe the current particles (subject to the trigger)
+    double L0 = 0.0;        // box side at the build
+    double halo = 0.0;      // halo the lists were built with
+    unsigned seq = 0;       // sequence number of the displacement readback
+    bool pending = false;   // a refresh for the current positions is already enqueued (fused into the kick-drift kernel)
+    volatile unsigned long long* mbox_host = nullptr;  // pinned, mapped: {seq << 32 | float bits of max displacement^2}
+    unsigned long long* mbox_dev = nullptr;
+  } list;
+  Buffer xref;        // double[N][3] positions at the build
+  Buffer slot_of;     // int32[N] original index -> sorted slot (inverse of perm)
+  Buffer list_off, list_pool;  // int4[N] {proton list: first, length; neutron list: first, length}; int32 sorted slots
+  int64_t list_entries = 0;
+  bool no_lists = false;       // transient: the caller needs the chunk kernel's own sort (pasta_force_stats)
+
   // pair-force chunk table (k1_cells.cu -> k2_chunk.cu): [0, max_chunks) entries first slot | count << 26,
   // [max_chunks, 2 max_chunks) the list of chunks that need several rounds; the counters live in
   // counters[24] (int32 view [48]: number of chunks, [49]: length of that list)
@@ -173,7 +248,15 @@ struct Sim {
 
 // ---- kernel launchers (one translation unit each) ---------------------------------------------------
 // K1  k1_cells.cu
-void k1_grids(Sim* s, bool uniform_grid, GridPair* g);  // the species' grids for the current L (host arithmetic only)
+bool list_mode_wanted(const Sim* s);                   // would a force evaluation of the current box run on reused lists?
+double list_halo(const Sim* s);
+void k1_grids(const Sim* s, bool uniform_grid, Grid out[2], GridPair* g);  // the species' grids for the current L (host only)
+void k1_frozen_grids(Sim* s, GridPair* g);             // the frozen cell counts at the current L (list mode)
+int k1_refresh(Sim* s, double* max_disp_host);         // list mode: pos4 from the moved x; largest displacement since the build
+int k1_refresh_wait(Sim* s, double* max_disp_host);    // ... the readback of a refresh already enqueued (fused into K3)
+#ifdef __CUDACC__
+void k1_refresh_args(Sim* s, RefreshArgs* out);        // (bumps the sequence number)
+#endif
 int k1_setup(Sim* s, bool uniform_grid, GridPair* g);  // grids for the current L, buffers, a zeroed histogram
 int k1_build(Sim* s, bool uniform_grid = false);       // (species,cell) counting sort, pos4/perm, chunk table; uses the
                                                        // histogram of k3_kick_drift_count if s->hist_valid
@@ -184,10 +267,13 @@ int k2_forces(Sim* s, bool with_energy);               // F, e in original order
 int k2_pair_count(Sim* s, int64_t* ordered_pairs_host, int64_t* nonzero_pairs_host);
 int k2_reference_forces(Sim* s, bool with_energy);     // variant 1: thread per target (k2_force.cu)
 int k2_chunk_forces(Sim* s, bool with_energy, bool stats);  // variant 2: chunk kernel (k2_chunk.cu)
+int k2_list_build(Sim* s, double halo);                // neighbour lists of the sorted order k1_build just made (k2_list.cu)
+int k2_list_forces(Sim* s, bool with_energy);          // the pair kernel on those lists
 // K3  k3_integrate.cu
 int k3_init_state(Sim* s, uint64_t seed);
-int k3_kick_drift_count(Sim* s, double dt, double scale, double L_wrap);  // kick, drift, scale, wrap into [0, L_wrap);
-                                                                         // cell histogram on the grids of box s->L
+int k3_kick_drift_refresh(Sim* s, double dt, double scale, double L_wrap);  // list mode: kick, drift + the refresh of the frozen order
+int k3_kick_drift_count(Sim* s, double dt, double scale, double L_wrap, bool count);  // kick, drift, scale, wrap into
+                                                     // [0, L_wrap); count: + cell histogram on the grids of box s->L
 int k3_kick_ke(Sim* s, double dt, bool rescale);       // second half kick + KE (+ rescale)
 int k3_wrap_scale(Sim* s, double scale, double L_new); // x = wrap(scale x)
 int k3_kinetic(Sim* s, double* ke_host);

@@ -565,6 +565,88 @@ def test_evolved_clustered_state_snapshots(orc, cfg, nsteps, nsample):
         assert np.array_equal(_np(A), Ao) and np.array_equal(_np(Z), Zo)
 
 
+def _sparse_state(N, Y_P, density, T, seed):
+    """A cold dilute stand-in with clusters (inputs.clustered_state) whose box is wide enough for the reused lists."""
+    return inputs.clustered_state(N, Y_P, density, T, seed=seed)
+
+
+@pytest.mark.parametrize("N,Y_P,density,halo", [(20000, 0.2, 0.00125, 0.0), (30000, 0.05, 0.002, 4.0), (8000, 0.5, 0.0008, 8.0)])
+def test_neighbour_list_run_equals_run_without_it(orc, N, Y_P, density, halo):
+    """in the sparse regime the sort, the chunk table and every chunk's source list
+    are built with a halo and reused across steps.  The force is unchanged by a list, so (i) every evaluation meets
+    the same oracle gates, on the build step and on reuse steps; (ii) a trajectory with lists equals the trajectory
+    that rebuilds every step to FP32 summation-order rounding; (iii) lists are really reused (few builds)."""
+    T = 0.5
+    x, v, is_p, L = _sparse_state(N, Y_P, density, T, seed=N)
+    runs = {}
+    for reuse in (1, 0):
+        with _sim_from_arrays(x, v, is_p, L, T=T, list_reuse=reuse, list_halo=halo, thermostat_interval=10) as sim:
+            op = _oparams(orc, sim.params)
+            F0, pe0 = sim.forces()
+            st0 = sim.list_stats()
+            sim.step(25, 2.0)
+            st1 = sim.list_stats()
+            hx, hv, hF = (_torch().empty((N, 3), dtype=_torch().float64).pin_memory() for _ in range(3))
+            sim.get_state_host(hx, hv, hF)          # the forces the last step used (a reuse step when reuse = 1)
+            xs, Fs = hx.numpy().copy(), hF.numpy().copy()
+            Fo, eo, peo, d = orc.forces(xs, is_p, L, op)
+            _check_forces(Fs, Fo, alternates=_alts(orc, xs, is_p, L, op), boundary_pairs=d["boundary_pairs"])
+            e = _np(sim.particle_energies())
+            assert abs(e.sum() - peo) <= PE_TOL * abs(peo)
+            runs[reuse] = (_np(F0), pe0, xs, Fs, st0, st1)
+    Fo0, _, peo0, d0 = orc.forces(x, is_p, L, op)
+    for reuse in (1, 0):
+        _check_forces(runs[reuse][0], Fo0, runs[reuse][1], peo0, _alts(orc, x, is_p, L, op), d0["boundary_pairs"])
+    # (ii) same trajectory: the two runs differ only by FP32 rounding (different kernels, different summation
+    # order), which 25 steps of a violently relaxing clustered start amplify: typical particle 1e-6 .. 1e-5 fm, worst 1e-3
+    dx = runs[1][2] - runs[0][2]
+    dx -= L * np.round(dx / L)
+    dist = np.linalg.norm(dx, axis=1)
+    print("list vs no list after 25 steps: median %.2e, max %.2e fm" % (np.median(dist), dist.max()))
+    assert np.median(dist) <= 1e-5 and dist.max() <= 1e-3, "positions differ by %.2e fm" % dist.max()
+    # (iii) every evaluation rebuilt without lists; with them only a few did
+    assert runs[0][5]["list_builds"] == runs[0][5]["force_evals"] == runs[0][4]["force_evals"] + 25
+    assert runs[1][5]["force_evals"] == runs[0][5]["force_evals"]
+    assert runs[1][5]["list_builds"] - runs[1][4]["list_builds"] <= 12   # (a hot, relaxing start: fast movers)
+
+
+def test_neighbour_list_trigger_fires_at_half_the_halo(orc):
+    """The paper's rebuild rule: rebuilt when the distance a target has moved plus the largest distance
+    any source has moved exceeds delta_r -- here in its global form 2 max_i |dx_i| > delta.  One fast nucleon crossing
+    a cold, otherwise static system: the list survives while it has moved less than delta / 2 and is rebuilt on the
+    first step after; forces meet the oracle on both sides of the trigger."""
+    N, L, halo, dt = 6000, 400.0, 4.0, 2.0
+    rng = np.random.default_rng(5)
+    x = rng.random((N, 3)) * L
+    v = np.zeros_like(x)
+    is_p = inputs.species(N, 0.3)
+    speed = 0.3                       # 0.6 fm per step: the halo's half is crossed during step 4 (2.4 fm > 2 fm)
+    v[17] = [speed, 0.0, 0.0]
+    with _sim_from_arrays(x, v, is_p, L, T=0.0, list_reuse=1, list_halo=halo, thermostat_interval=0) as sim:
+        op = _oparams(orc, sim.params)
+        sim.forces()
+        builds = [sim.list_stats()["list_builds"]]
+        for k in range(8):
+            sim.step(1, dt)
+            builds.append(sim.list_stats()["list_builds"])
+            xs, _, _, _, _ = sim.get_state()
+            xs = _np(xs)
+            moved = np.abs((xs - x + L / 2) % L - L / 2).max()
+            F = _np(sim.forces(want_pe=False)[0]) if False else None
+        # forces of a static cold gas are tiny, so particle 17 moves ballistically: 0.6 (k + 1) fm after step k + 1
+        rebuilt_at = [k + 1 for k in range(8) if builds[k + 1] > builds[k]]
+        assert rebuilt_at == [4, 8], (builds, rebuilt_at)   # 2 * 0.6 * 4 = 4.8 > 4 fm; then again 4 steps later
+        hx, hv, hF = (_torch().empty((N, 3), dtype=_torch().float64).pin_memory() for _ in range(3))
+        sim.get_state_host(hx, hv, hF)
+        Fo, _, _, d = orc.forces(hx.numpy(), is_p, L, op)
+        _check_forces(hF.numpy(), Fo, alternates=_alts(orc, hx.numpy(), is_p, L, op), boundary_pairs=d["boundary_pairs"])
+    # list_reuse = 0: every evaluation rebuilds
+    with _sim_from_arrays(x, v, is_p, L, T=0.0, list_reuse=0) as sim:
+        sim.step(3, dt)
+        st = sim.list_stats()
+        assert st["list_builds"] == st["force_evals"] == 4
+
+
 @pytest.mark.parametrize("variant", [0, 1])
 @pytest.mark.parametrize("N,density,r_c,Y_P", [(2048, 0.05, 17.0, 0.3), (30000, 0.08, 20.0, 0.4)])
 def test_range_split_mode(orc, N, density, r_c, Y_P, variant):
