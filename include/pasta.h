@@ -166,6 +166,25 @@ int pasta_set_state_host(pasta_sim* sim, const double* x_host, const double* v_h
                          const double* F_host, double L);
 
 /*
+ * Pipelined host transfers.  The same state exchange as pasta_set_state_host / pasta_get_state_host, but on two side
+ * streams with double-buffered device staging, so that while step k is being computed the inputs of step k + 1 are
+ * already crossing PCIe in one direction and the result of step k - 1 in the other.  Both calls return at once.
+ *   pasta_set_state_host_async: x, v, F (F may be NULL: forces stale) are copied host -> staging on the upload stream;
+ *     the simulation's stream then takes them over (device copy, wrap into [0, L)).  The host buffers may be reused
+ *     after the NEXT BUT ONE async set, or after pasta_host_sync.
+ *   pasta_get_state_host_async: the simulation's stream snapshots x, v, F into staging (forces evaluated first if
+ *     stale); the download stream copies the snapshot to the host buffers, which are valid after pasta_host_sync (or
+ *     after the next but one async get has returned and been synchronised).  L and the step count are returned at once
+ *     (the host tracks them).
+ *   pasta_host_sync: waits for the simulation's stream and both side streams.
+ * Use pinned host memory; pageable memory makes the copies synchronous.
+ */
+int pasta_set_state_host_async(pasta_sim* sim, const double* x_host, const double* v_host, const double* F_host, double L);
+int pasta_get_state_host_async(pasta_sim* sim, double* x_host, double* v_host, double* F_host, double* L_host,
+                               int64_t* step_host);
+int pasta_host_sync(pasta_sim* sim);
+
+/*
  * Cell assignment of the current positions on the species-independent grid of pasta_params.cell_subdiv
  * (D14) -- NOT the grids the force kernel sorts on, see pasta_force_cells below:
  *   ncell = max(1, floor(L k / r_c)); c = min(ncell-1, floor(x * (ncell/L))) per axis (FP64);

@@ -61,6 +61,10 @@ SIGNATURES = {
     "pasta_get_state_host": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.POINTER(C.c_double),
                                        C.POINTER(C.c_int64)]),
     "pasta_set_state_host": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_double]),
+    "pasta_set_state_host_async": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_double]),
+    "pasta_get_state_host_async": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.POINTER(C.c_double),
+                                             C.POINTER(C.c_int64)]),
+    "pasta_host_sync": (C.c_int, [C.c_void_p]),
     "pasta_cells": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.POINTER(C.c_int32)]),
     "pasta_ncell": (C.c_int, [C.c_void_p, C.POINTER(C.c_int32)]),
     "pasta_force_grid": (C.c_int, [C.c_void_p, C.POINTER(C.c_int32)]),
@@ -267,6 +271,23 @@ class Sim:
         L, step = C.c_double(), C.c_int64()
         _check(self.lib.pasta_get_state_host(self._h, hp(x), hp(v), hp(F), C.byref(L), C.byref(step)))
         return L.value, step.value
+
+    def set_state_host_async(self, x, v, F=None, L=None):
+        """Pipelined upload (pinned torch CPU tensors): returns at once; see pasta_set_state_host_async."""
+        if L is None:
+            L = self.box_length()
+        hp = lambda t: None if t is None else C.c_void_p(t.data_ptr())  # noqa: E731
+        _check(self.lib.pasta_set_state_host_async(self._h, hp(x), hp(v), hp(F), float(L)))
+
+    def get_state_host_async(self, x=None, v=None, F=None):
+        """Pipelined download: returns (L, step) at once; the buffers are valid after host_sync()."""
+        hp = lambda t: None if t is None else C.c_void_p(t.data_ptr())  # noqa: E731
+        L, step = C.c_double(), C.c_int64()
+        _check(self.lib.pasta_get_state_host_async(self._h, hp(x), hp(v), hp(F), C.byref(L), C.byref(step)))
+        return L.value, step.value
+
+    def host_sync(self):
+        _check(self.lib.pasta_host_sync(self._h))
 
     def box_length(self):
         L = C.c_double()

@@ -321,6 +321,20 @@ int pasta_destroy(pasta_sim* sim) {
   if (!s) return PASTA_OK;
   cudaSetDevice(s->env.device);
   cudaStreamSynchronize(s->stream);
+  if (s->pipe.up) {
+    cudaStreamSynchronize(s->pipe.up);
+    cudaStreamSynchronize(s->pipe.down);
+    for (int b = 0; b < 2; ++b) {
+      buffer_release(s, &s->pipe.in[b]);
+      buffer_release(s, &s->pipe.out[b]);
+      cudaEventDestroy(s->pipe.in_done[b]);
+      cudaEventDestroy(s->pipe.in_taken[b]);
+      cudaEventDestroy(s->pipe.out_ready[b]);
+      cudaEventDestroy(s->pipe.out_done[b]);
+    }
+    cudaStreamDestroy(s->pipe.up);
+    cudaStreamDestroy(s->pipe.down);
+  }
   release_all(s);
   if (s->list.mbox_host) cudaFreeHost(const_cast<unsigned long long*>(s->list.mbox_host));
   for (cudaEvent_t e : s->evs)
@@ -532,6 +546,90 @@ int pasta_get_state_host(pasta_sim* sim, double* x_host, double* v_host, double*
   if (L_host) *L_host = s->L;
   if (step_host) *step_host = s->step_count;
   PASTA_CUDA_OK(cudaStreamSynchronize(s->stream));
+  return PASTA_OK;
+}
+
+static int pipe_setup(Sim* s) {
+  Sim::HostPipe& p = s->pipe;
+  if (p.up) return PASTA_OK;
+  PASTA_CUDA_OK(cudaStreamCreateWithFlags(&p.up, cudaStreamNonBlocking));
+  PASTA_CUDA_OK(cudaStreamCreateWithFlags(&p.down, cudaStreamNonBlocking));
+  for (int b = 0; b < 2; ++b) {
+    PASTA_TRY(buffer_reserve(s, &p.in[b], 72 * (size_t)s->N));
+    PASTA_TRY(buffer_reserve(s, &p.out[b], 72 * (size_t)s->N));
+    PASTA_CUDA_OK(cudaEventCreateWithFlags(&p.in_done[b], cudaEventDisableTiming));
+    PASTA_CUDA_OK(cudaEventCreateWithFlags(&p.in_taken[b], cudaEventDisableTiming));
+    PASTA_CUDA_OK(cudaEventCreateWithFlags(&p.out_ready[b], cudaEventDisableTiming));
+    PASTA_CUDA_OK(cudaEventCreateWithFlags(&p.out_done[b], cudaEventDisableTiming));
+  }
+  return PASTA_OK;
+}
+
+int pasta_set_state_host_async(pasta_sim* sim, const double* x_host, const double* v_host, const double* F_host, double L) {
+  Sim* s = reinterpret_cast<Sim*>(sim);
+  PASTA_TRY(check_sim(s));
+  if (!x_host || !v_host || !(L > 0.0) || s->prm.r_c > 0.5 * L) {
+    set_error("pasta_set_state_host_async: need x, v and L >= 2 r_c");
+    return PASTA_EINVAL;
+  }
+  PASTA_TRY(use_device(s));
+  PASTA_TRY(pipe_setup(s));
+  Sim::HostPipe& p = s->pipe;
+  const int b = (int)(p.n_in & 1);
+  const size_t n = 24 * (size_t)s->N;
+  char* st = p.in[b].as<char>();
+  // upload stream: the staging buffer is free once the simulation's stream has taken the upload before last
+  if (p.n_in >= 2) PASTA_CUDA_OK(cudaStreamWaitEvent(p.up, p.in_taken[b], 0));
+  PASTA_CUDA_OK(cudaMemcpyAsync(st, x_host, n, cudaMemcpyHostToDevice, p.up));
+  PASTA_CUDA_OK(cudaMemcpyAsync(st + n, v_host, n, cudaMemcpyHostToDevice, p.up));
+  if (F_host) PASTA_CUDA_OK(cudaMemcpyAsync(st + 2 * n, F_host, n, cudaMemcpyHostToDevice, p.up));
+  PASTA_CUDA_OK(cudaEventRecord(p.in_done[b], p.up));
+  // simulation's stream: take the state over
+  PASTA_CUDA_OK(cudaStreamWaitEvent(s->stream, p.in_done[b], 0));
+  PASTA_CUDA_OK(cudaMemcpyAsync(s->x.ptr, st, n, cudaMemcpyDeviceToDevice, s->stream));
+  PASTA_CUDA_OK(cudaMemcpyAsync(s->v.ptr, st + n, n, cudaMemcpyDeviceToDevice, s->stream));
+  if (F_host) PASTA_CUDA_OK(cudaMemcpyAsync(s->F.ptr, st + 2 * n, n, cudaMemcpyDeviceToDevice, s->stream));
+  PASTA_CUDA_OK(cudaEventRecord(p.in_taken[b], s->stream));
+  p.n_in += 1;
+  return after_set_state(s, false, F_host != nullptr, L);
+}
+
+int pasta_get_state_host_async(pasta_sim* sim, double* x_host, double* v_host, double* F_host, double* L_host,
+                               int64_t* step_host) {
+  Sim* s = reinterpret_cast<Sim*>(sim);
+  PASTA_TRY(check_sim(s));
+  PASTA_TRY(use_device(s));
+  PASTA_TRY(pipe_setup(s));
+  Sim::HostPipe& p = s->pipe;
+  const int b = (int)(p.n_out & 1);
+  const size_t n = 24 * (size_t)s->N;
+  char* st = p.out[b].as<char>();
+  if (F_host && !s->forces_valid) PASTA_TRY(evaluate_forces(s, s->prm.energy_every_step != 0));
+  // simulation's stream: snapshot (the staging buffer is free once the download before last has left it)
+  if (p.n_out >= 2) PASTA_CUDA_OK(cudaStreamWaitEvent(s->stream, p.out_done[b], 0));
+  if (x_host) PASTA_CUDA_OK(cudaMemcpyAsync(st, s->x.ptr, n, cudaMemcpyDeviceToDevice, s->stream));
+  if (v_host) PASTA_CUDA_OK(cudaMemcpyAsync(st + n, s->v.ptr, n, cudaMemcpyDeviceToDevice, s->stream));
+  if (F_host) PASTA_CUDA_OK(cudaMemcpyAsync(st + 2 * n, s->F.ptr, n, cudaMemcpyDeviceToDevice, s->stream));
+  PASTA_CUDA_OK(cudaEventRecord(p.out_ready[b], s->stream));
+  // download stream
+  PASTA_CUDA_OK(cudaStreamWaitEvent(p.down, p.out_ready[b], 0));
+  if (x_host) PASTA_CUDA_OK(cudaMemcpyAsync(x_host, st, n, cudaMemcpyDeviceToHost, p.down));
+  if (v_host) PASTA_CUDA_OK(cudaMemcpyAsync(v_host, st + n, n, cudaMemcpyDeviceToHost, p.down));
+  if (F_host) PASTA_CUDA_OK(cudaMemcpyAsync(F_host, st + 2 * n, n, cudaMemcpyDeviceToHost, p.down));
+  PASTA_CUDA_OK(cudaEventRecord(p.out_done[b], p.down));
+  p.n_out += 1;
+  if (L_host) *L_host = s->L;
+  if (step_host) *step_host = s->step_count;
+  return PASTA_OK;
+}
+
+int pasta_host_sync(pasta_sim* sim) {
+  Sim* s = reinterpret_cast<Sim*>(sim);
+  PASTA_TRY(check_sim(s));
+  PASTA_TRY(use_device(s));
+  PASTA_CUDA_OK(cudaStreamSynchronize(s->stream));
+  if (s->pipe.up) PASTA_CUDA_OK(cudaStreamSynchronize(s->pipe.up));
+  if (s->pipe.down) PASTA_CUDA_OK(cudaStreamSynchronize(s->pipe.down));
   return PASTA_OK;
 }
 

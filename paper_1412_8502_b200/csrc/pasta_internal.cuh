@@ -237,6 +237,15 @@ struct Sim {
   int64_t chunk_nprim = 0;
   bool chunks_sparse = false;  // some species' chunks come from the SPARSE (cell block) builder
 
+  // pipelined host transfers (pasta_*_host_async): side streams, double-buffered staging, hand-over events
+  struct HostPipe {
+    cudaStream_t up = nullptr, down = nullptr;
+    Buffer in[2], out[2];                 // 72 N bytes each: x, v, F
+    cudaEvent_t in_done[2] = {nullptr, nullptr}, in_taken[2] = {nullptr, nullptr};
+    cudaEvent_t out_ready[2] = {nullptr, nullptr}, out_done[2] = {nullptr, nullptr};
+    int64_t n_in = 0, n_out = 0;
+  } pipe;
+
   // timing: pairs of events (start, stop) tagged with the kernel group they bracket
   bool timing = false;
   std::vector<cudaEvent_t> evs;

@@ -380,6 +380,35 @@ def test_restart_with_forces_and_host_buffers(orc):
         c1.close()
 
 
+def test_pipelined_host_transfers_equal_the_blocking_ones():
+    """pasta_set/get_state_host_async (the e2e leg of bench.py): side-stream copies with double-buffered staging give
+    bit-identical results to the blocking calls, for independent requests issued back to back without any sync."""
+    torch = _torch()
+    N = 20000
+    states = [inputs.uniform_state(N, 0.3, 0.06, 1.0, seed=40 + k) for k in range(5)]
+    L = states[0][3]
+    pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()  # noqa: E731
+    with _sim_from_arrays(*states[0][:3], L, r_c=15.0) as sim:
+        want = []
+        for x, v, is_p, _ in states:
+            sim.set_state_host(pin(x), pin(v), None, None, L)
+            sim.step(2, 2.0)
+            out = [torch.empty((N, 3), dtype=torch.float64).pin_memory() for _ in range(3)]
+            sim.get_state_host(*out)
+            want.append([o.clone() for o in out])
+        ins = [(pin(x), pin(v)) for x, v, _, _ in states]
+        outs = [[torch.empty((N, 3), dtype=torch.float64).pin_memory() for _ in range(3)] for _ in states]
+        for k in range(len(states)):
+            sim.set_state_host_async(ins[k][0], ins[k][1], None, L)
+            sim.step(2, 2.0)
+            Lk, stepk = sim.get_state_host_async(*outs[k])
+            assert Lk == L
+        sim.host_sync()
+        for k in range(len(states)):
+            for a, b in zip(outs[k], want[k]):
+                assert torch.equal(a, b), "request %d differs" % k
+
+
 def test_device_initial_state_statistics():
     """P15 on the device generator: uniform positions, normal velocities with variance T/M (D15)."""
     N, T = 200000, 0.5
