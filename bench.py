@@ -252,7 +252,6 @@ def run_ours(args, rank, world, local_rank):
     for _ in range(max(args.warmup, 3)):
         sim.step(1, c["dt"])
     torch.cuda.synchronize()
-    sim.set_timing(True)
     n0 = sim.launch_count()
     ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
     barrier()
@@ -265,8 +264,15 @@ def run_ours(args, rank, world, local_rank):
         b.record()
     barrier()
     t_wall = time.perf_counter() - t_wall0
-    clocks = sampler.stop() if sampler else None
     launches = sim.launch_count() - n0
+    # ---- the same steps once more with the library's own event brackets around the kernel groups (K1 / K2 / K3): the
+    # brackets switch the captured-graph replay of a step off, so they are kept out of the headline region above
+    sim.set_timing(True)
+    for _ in range(min(args.steps, 200)):
+        flush.zero_()
+        sim.step(1, c["dt"])
+    barrier()
+    clocks = sampler.stop() if sampler else None
     tm = sim.get_timing()
     sim.set_timing(False)
     per_step_ms = sorted(a.elapsed_time(b) for a, b in ev)

@@ -237,6 +237,13 @@ int pasta_list_stats(pasta_sim* sim, int64_t* out2_host);
 int pasta_set_timing(pasta_sim* sim, int32_t enable);
 int pasta_get_timing(pasta_sim* sim, double* ms3_host, int64_t* n_force_evals_host);
 int64_t pasta_launch_count(const pasta_sim* sim);
+/* A step in a fixed box (scale_per_step == 1, xi_dot == 0) on the chunk path enqueues the same kernels with the same
+ * arguments every time; after two such steps pasta_step captures it as a CUDA graph (one for a plain step, one for a
+ * step that ends with the velocity rescale) and replays it with a single launch.  Timing brackets, a
+ * scaling box, the neighbour-list regime, a new particle set or dt, or PASTA_GRAPHS=0 in the environment take the
+ * kernel-by-kernel path; the results are bit-identical either way.  Returns the number of steps replayed so far
+ * (pasta_launch_count counts the kernels inside a replayed step as launched). */
+int64_t pasta_graph_replays(const pasta_sim* sim);
 
 const char* pasta_last_error(void);
 const char* pasta_version(void);

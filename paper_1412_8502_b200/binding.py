@@ -78,6 +78,7 @@ SIGNATURES = {
     "pasta_set_timing": (C.c_int, [C.c_void_p, C.c_int32]),
     "pasta_get_timing": (C.c_int, [C.c_void_p, C.POINTER(C.c_double), C.POINTER(C.c_int64)]),
     "pasta_launch_count": (C.c_int64, [C.c_void_p]),
+    "pasta_graph_replays": (C.c_int64, [C.c_void_p]),
     "pasta_last_error": (C.c_char_p, []),
     "pasta_version": (C.c_char_p, []),
 }
@@ -377,3 +378,6 @@ class Sim:
 
     def launch_count(self):
         return int(self.lib.pasta_launch_count(self._h))
+
+    def graph_replays(self):
+        return int(self.lib.pasta_graph_replays(self._h))

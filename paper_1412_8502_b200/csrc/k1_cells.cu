@@ -539,6 +539,7 @@ int k1_build(Sim* s, bool uniform_grid) {
         s->launches += 1;
       }
   }
+  s->sort_kind = uniform ? 1 : (lists ? 2 : 0);
   PASTA_CUDA_OK(cudaGetLastError());
   return PASTA_OK;
 }
@@ -618,6 +619,7 @@ int k1_export_cells(Sim* s, int32_t* cell_id_dev, int32_t* cell_start_dev) {
   const Grid g = make_grid(s->L, s->prm.r_c, s->prm.cell_subdiv);
   s->hist_valid = false;  // cell_id and the histogram table are about to hold the exported grid
   s->bins_zeroed = 0;
+  s->sort_kind = -1;
   PASTA_TRY(buffer_reserve(s, &s->bin_count, sizeof(int32_t) * (size_t)(g.nc3 + 1)));
   PASTA_TRY(buffer_reserve(s, &s->bin_start, sizeof(int32_t) * (size_t)(g.nc3 + 1)));
   int32_t* cnt = s->bin_count.as<int32_t>();

@@ -39,6 +39,7 @@ int buffer_reserve(Sim* s, Buffer* b, size_t bytes) {
   }
   b->ptr = p;
   b->bytes = want;
+  s->state_gen += 1;  // a captured step holds the old pointer
   return PASTA_OK;
 }
 
@@ -162,6 +163,125 @@ static int evaluate_forces(Sim* s, bool with_energy) {
   return evaluate_forces_tail(s, with_energy);
 }
 
+// One MD step with s->L already set to the box the forces are evaluated in (O2: first half kick + drift, forces,
+// second half kick, rescale on every thermostat_interval-th step).
+static int step_body(Sim* s, double dt, double sc, double L_wrap, bool energy, bool rescale) {
+  {
+    Timer t(s, 2);
+    // the cell histogram of the new positions rides along unless the sorted order is frozen (or about to be
+    // rebuilt on the lists' own grid)
+    if (s->list.valid) PASTA_TRY(k3_kick_drift_refresh(s, dt, sc, L_wrap));
+    else PASTA_TRY(k3_kick_drift_count(s, dt, sc, L_wrap, !list_mode_wanted(s)));
+    s->lin_n += 1;
+  }
+  s->clusters_valid = false;
+  PASTA_TRY(evaluate_forces(s, energy));
+  s->step_count += 1;
+  {
+    Timer t(s, 2);
+    PASTA_TRY(k3_kick_ke(s, dt, rescale));
+  }
+  return PASTA_OK;
+}
+
+static void graphs_drop(Sim* s) {
+  for (int w = 0; w < 2; ++w) {
+    if (s->graph.exec[w]) cudaGraphExecDestroy(s->graph.exec[w]);
+    s->graph.exec[w] = nullptr;
+  }
+  s->graph.gen = -1;
+  s->graph.warm = 0;
+}
+static void graphs_destroy(Sim* s) {
+  graphs_drop(s);
+  if (s->graph.cap) cudaStreamDestroy(s->graph.cap);
+  s->graph.cap = nullptr;
+}
+
+// A fixed-box step on the chunk path enqueues the same 8-10 kernels with the same arguments every time (SURVEY 3b:
+// "capture the step in a CUDA graph"): after two such steps have run kernel by kernel (every buffer has its final size
+// by then) the step is captured once per kind (plain / ending with the rescale) and replayed with one launch.
+// Anything that changes a captured argument -- a buffer that moved, a new particle set, another dt or box -- drops
+// the graphs; timing brackets, a scaling box and the neighbour-list regime always take the kernel-by-kernel path.
+static int step_once(Sim* s, double dt, double sc, double L_wrap, bool energy, bool rescale) {
+  const bool eligible = s->tune.graphs != 0 && sc == 1.0 && !(s->prm.xi_dot > 0.0) && !s->timing && !s->list.valid &&
+                        s->tune.force_variant == 0 && s->forces_valid && !list_mode_wanted(s) && s->sort_kind == 0 &&
+                        s->bins_zeroed >= s->grid_sp[0].nc3 + s->grid_sp[1].nc3 + 1;
+  if (!eligible) {
+    s->graph.warm = 0;
+    return step_body(s, dt, sc, L_wrap, energy, rescale);
+  }
+  if (s->graph.gen != s->state_gen || s->graph.L != s->L || s->graph.dt != dt || s->graph.energy != (int)energy) {
+    graphs_drop(s);
+    s->graph.gen = s->state_gen;
+    s->graph.L = s->L;
+    s->graph.dt = dt;
+    s->graph.energy = (int)energy;
+  }
+  const int w = rescale ? 1 : 0;
+  if (!s->graph.exec[w]) {
+    if (s->graph.warm < 2) {
+      s->graph.warm += 1;
+      const int rc = step_body(s, dt, sc, L_wrap, energy, rescale);
+      if (s->graph.gen != s->state_gen) s->graph.warm = 0;  // a buffer grew during this step: not settled yet
+      return rc;
+    }
+    // capture this step; the host-side bookkeeping of step_body runs now, its kernels when the graph is launched
+    const int64_t launches0 = s->launches;
+    if (!s->graph.cap && cudaStreamCreateWithFlags(&s->graph.cap, cudaStreamNonBlocking) != cudaSuccess) s->graph.cap = nullptr;
+    if (!s->graph.cap || cudaStreamBeginCapture(s->graph.cap, cudaStreamCaptureModeThreadLocal) != cudaSuccess) {
+      cudaGetLastError();
+      s->tune.graphs = 0;
+      return step_body(s, dt, sc, L_wrap, energy, rescale);
+    }
+    cudaStream_t const user_stream = s->stream;
+    s->stream = s->graph.cap;
+    const int rc = step_body(s, dt, sc, L_wrap, energy, rescale);
+    s->stream = user_stream;
+    cudaGraph_t g = nullptr;
+    const cudaError_t ce = cudaStreamEndCapture(s->graph.cap, &g);
+    if (rc != PASTA_OK || ce != cudaSuccess || !g || s->graph.gen != s->state_gen) {
+      if (g) cudaGraphDestroy(g);
+      cudaGetLastError();
+      s->tune.graphs = 0;
+      s->forces_valid = false;  // the captured kernels never ran: positions, velocities and forces are those of the
+      s->hist_valid = false;    // step before; undo the bookkeeping and redo the step kernel by kernel
+      s->bins_zeroed = 0;
+      s->step_count -= 1;
+      s->lin_n -= 1;
+      s->n_force_evals -= 1;
+      s->n_list_builds -= 1;
+      s->launches = launches0;
+      if (rc != PASTA_OK) return rc;
+      PASTA_TRY(evaluate_forces(s, energy));
+      return step_body(s, dt, sc, L_wrap, energy, rescale);
+    }
+    const cudaError_t ie = cudaGraphInstantiate(&s->graph.exec[w], g, 0);
+    cudaGraphDestroy(g);
+    if (ie != cudaSuccess) {
+      set_error("cudaGraphInstantiate failed: %s", cudaGetErrorString(ie));
+      return PASTA_ECUDA;
+    }
+    s->graph.launches[w] = s->launches - launches0;
+    PASTA_CUDA_OK(cudaGraphLaunch(s->graph.exec[w], s->stream));
+    s->graph.replays += 1;
+    return PASTA_OK;
+  }
+  // replay: the bookkeeping of step_body, then one launch
+  PASTA_CUDA_OK(cudaGraphLaunch(s->graph.exec[w], s->stream));
+  s->lin_n += 1;
+  s->step_count += 1;
+  s->clusters_valid = false;
+  s->n_force_evals += 1;
+  s->n_list_builds += 1;
+  s->hist_valid = false;
+  s->forces_valid = true;
+  s->energies_valid = energy;
+  s->launches += s->graph.launches[w];
+  s->graph.replays += 1;
+  return PASTA_OK;
+}
+
 }  // namespace pasta
 
 using namespace pasta;
@@ -255,6 +375,7 @@ int pasta_create(pasta_sim** out, int64_t N, double Y_P, double density, double 
     s->tune.force_variant = env_int("PASTA_FORCE_VARIANT", 0);
     s->tune.auto_grid = env_int("PASTA_AUTO_GRID", 1);
     s->tune.x_subdiv = env_int("PASTA_X_SUBDIV", 0);
+    s->tune.graphs = env_int("PASTA_GRAPHS", 1);
   }
   if (env) {
     s->env = *env;
@@ -321,6 +442,7 @@ int pasta_destroy(pasta_sim* sim) {
   if (!s) return PASTA_OK;
   cudaSetDevice(s->env.device);
   cudaStreamSynchronize(s->stream);
+  graphs_destroy(s);
   if (s->pipe.up) {
     cudaStreamSynchronize(s->pipe.up);
     cudaStreamSynchronize(s->pipe.down);
@@ -379,22 +501,8 @@ int pasta_step(pasta_sim* sim, int64_t n, double dt) {
       return PASTA_EINVAL;
     }
     s->L = L_new;
-    {
-      Timer t(s, 2);
-      // the cell histogram of the new positions rides along unless the sorted order is frozen (or about to be
-      // rebuilt on the lists' own grid)
-      if (s->list.valid) PASTA_TRY(k3_kick_drift_refresh(s, dt, sc, linear ? L_old : L_new));
-      else PASTA_TRY(k3_kick_drift_count(s, dt, sc, linear ? L_old : L_new, !list_mode_wanted(s)));
-      s->lin_n += 1;
-    }
-    s->clusters_valid = false;
-    PASTA_TRY(evaluate_forces(s, energy));
-    s->step_count += 1;
-    const bool rescale = s->prm.thermostat_interval > 0 && (s->step_count % s->prm.thermostat_interval) == 0;
-    {
-      Timer t(s, 2);
-      PASTA_TRY(k3_kick_ke(s, dt, rescale));
-    }
+    const bool rescale = s->prm.thermostat_interval > 0 && ((s->step_count + 1) % s->prm.thermostat_interval) == 0;
+    PASTA_TRY(step_once(s, dt, sc, linear ? L_old : L_new, energy, rescale));
   }
   return PASTA_OK;
 }
@@ -492,6 +600,7 @@ static int after_set_state(Sim* s, bool have_is_p, bool have_F, double L) {
   PASTA_TRY(k3_wrap_scale(s, 1.0, L));
   if (have_is_p) {
     PASTA_TRY(k3_count_protons(s));  // the sorted layout needs the new proton count on the host
+    s->state_gen += 1;               // ... and a captured step was built for the old one
   }
   s->forces_valid = have_F;
   s->energies_valid = false;
@@ -807,6 +916,11 @@ int pasta_get_timing(pasta_sim* sim, double* ms3_host, int64_t* n_force_evals_ho
 int64_t pasta_launch_count(const pasta_sim* sim) {
   const Sim* s = reinterpret_cast<const Sim*>(sim);
   return s ? s->launches : 0;
+}
+
+int64_t pasta_graph_replays(const pasta_sim* sim) {
+  const Sim* s = reinterpret_cast<const Sim*>(sim);
+  return s ? s->graph.replays : 0;
 }
 
 }  // extern "C"

@@ -163,6 +163,7 @@ struct Tuning {
   int force_variant = 0;  // 0 = chunk kernel (production); 1 = thread-per-target kernel on one isotropic grid (k2_force.cu)
   int auto_grid = 1;      // 1: each species' force grid picks its own k (about 8 particles per cell); 0: both use cell_subdiv
   int x_subdiv = 0;       // thin cells along x per force-grid cell (0 = automatic: 8, fewer for a sparse species)
+  int graphs = 1;         // replay a fixed-box step as a CUDA graph (PASTA_GRAPHS=0: always enqueue kernel by kernel)
 };
 
 struct Sim {
@@ -245,6 +246,20 @@ struct Sim {
     cudaEvent_t out_ready[2] = {nullptr, nullptr}, out_done[2] = {nullptr, nullptr};
     int64_t n_in = 0, n_out = 0;
   } pipe;
+
+  // a fixed-box MD step captured as a CUDA graph (pasta_step): [0] plain step, [1] step that ends with the rescale
+  struct StepGraph {
+    cudaGraphExec_t exec[2] = {nullptr, nullptr};
+    int64_t launches[2] = {0, 0};  // kernels in each
+    double L = 0.0, dt = 0.0;      // what the captured kernel arguments were computed for
+    int energy = 0;
+    int64_t gen = -1;              // value of state_gen at capture
+    int64_t replays = 0;           // steps replayed so far
+    cudaStream_t cap = nullptr;    // capture happens on a stream of our own (the caller's may be the legacy default stream)
+    int warm = 0;                  // eligible steps enqueued kernel by kernel since the last change (buffers settle)
+  } graph;
+  int sort_kind = -1;     // what the sorted arrays and grid_sp describe: 0 chunk-path grids, 1 uniform grid, 2 list grid, -1 nothing
+  int64_t state_gen = 0;  // bumped whenever a device buffer moves or the particle set changes: captured graphs are stale
 
   // timing: pairs of events (start, stop) tagged with the kernel group they bracket
   bool timing = false;

@@ -754,3 +754,41 @@ def test_random_small_systems(orc, seed):
     else:
         assert np.abs(_np(F)).max() == 0.0
     assert abs(pairs - d["ordered_pairs"]) <= 4
+
+
+def test_captured_step_equals_kernel_by_kernel(monkeypatch):
+    """a fixed-box step is captured as a CUDA graph after two warm steps and replayed with one launch.
+    The replay must (i) really happen, (ii) leave positions, velocities, forces and the kinetic energy BIT-identical to
+    the kernel-by-kernel path (PASTA_GRAPHS=0), across rescale steps (interval 10: both graphs are used), across a
+    foreign use of the sort buffers (pasta_cells, pasta_pair_count) and a state upload in between, and (iii) stop
+    when the box starts to scale."""
+    c = inputs.CONFIGS[1]
+    out = []
+    for graphs in ("1", "0"):
+        monkeypatch.setenv("PASTA_GRAPHS", graphs)
+        p = pasta.default_params(r_c=c["r_c"], thermostat_interval=10)
+        with pasta.Sim(8192, 0.3, 0.05, 1.0, params=p, seed=11) as sim:
+            sim.step(25, 2.0)
+            r0 = sim.graph_replays()
+            assert (r0 >= 20) if graphs == "1" else (r0 == 0)
+            sim.cells()                      # the exported O3 grid borrows the histogram buffers
+            sim.pair_count()                 # ... and the counting kernel re-sorts on one common grid
+            sim.step(3, 2.0)
+            x, v, is_p, L, step = sim.get_state()
+            sim.set_state(x, v, None, None, L)   # new positions, forces stale: one evaluation outside the graph
+            sim.step(12, 2.0)
+            assert step == 28 and sim.get_state()[4] == 40
+            if graphs == "1":
+                assert sim.graph_replays() > r0 + 8
+            F, pe = sim.forces()
+            x, v, _, L, _ = sim.get_state()
+            out.append((x.clone(), v.clone(), F.clone(), pe, sim.kinetic(), sim.launch_count()))
+    a, b = out
+    assert _torch().equal(a[0], b[0]) and _torch().equal(a[1], b[1]) and _torch().equal(a[2], b[2])
+    assert a[3] == b[3] and a[4] == b[4] and a[5] == b[5]
+    # a scaling box never replays
+    monkeypatch.setenv("PASTA_GRAPHS", "1")
+    p = pasta.default_params(r_c=c["r_c"], thermostat_interval=10, scale_per_step=1.0005)
+    with pasta.Sim(8192, 0.3, 0.05, 1.0, params=p, seed=11) as sim:
+        sim.step(12, 2.0)
+        assert sim.graph_replays() == 0
