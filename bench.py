@@ -194,13 +194,14 @@ def run_reference(args, rank, world):
     print(json.dumps(line), flush=True)
 
 
-def workload_config(cfg, world):
+def workload_config(cfg, world, sharded=False):
     c = inputs.CONFIGS[cfg]
     return {
         "workload": "BASELINE config %d: %d nucleons, Y_P=%.2f, n=%.3f fm^-3, T=%.2f MeV, r_c=%g fm, dt=%g fm/c, "
                     "velocity rescale every %d steps, seeded uniform-random start" % (
                         cfg, c["N"], c["Y_P"], c["density"], c["T"], c["r_c"], c["dt"], c["thermostat_interval"]),
-        "N": c["N"], "parallelism": "replicas x%d (one GPU each, no data-path collective)" % world,
+        "N": c["N"], "parallelism": ("one simulation, targets sharded over %d GPUs, force all-reduce (NCCL) per evaluation" % world)
+        if sharded else "replicas x%d (one GPU each, no data-path collective)" % world,
         "l2": "flushed between timed steps (256 MB write); the 50 MB MD state is otherwise L2-resident by nature",
     }
 
@@ -240,7 +241,12 @@ def run_ours(args, rank, world, local_rank):
     for kv in filter(None, args.params.split(",")):  # pasta_params overrides, e.g. --params r_nuc=11.5,skip_exact_zeros=0
         key, val = kv.split("=")
         setattr(prm, key, type(getattr(prm, key))(float(val)))
-    sim = pasta.Sim(N, c["Y_P"], c["density"], c["T"], params=prm, seed=args.seed + rank)
+    # replicas (default): rank r runs its own simulation (seed + r).  --shard: ONE simulation, replicated state, the
+    # targets of every force evaluation split over the ranks and the partial forces summed with an NCCL all-reduce
+    sharded = bool(args.shard) and world > 1
+    sim = pasta.Sim(N, c["Y_P"], c["density"], c["T"], params=prm, seed=args.seed + (0 if sharded else rank))
+    if sharded:
+        sim.set_shard(rank, world)
     flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")
 
     def barrier():
@@ -331,13 +337,13 @@ def run_ours(args, rank, world, local_rank):
         achieved = (17.0 * pairs_nz + 8.0 * c["Y_P"] ** 2 * pairs) / k2_s
         traffic, traffic_src = ncu_traffic(args.config)
         roof_pairs = min(fp32_peak / c_fp32, mufu_peak / c_mufu)
-        steps_per_s = aggregate_rate(world, args.steps, dev_s)
+        steps_per_s = aggregate_rate(1 if sharded else world, args.steps, dev_s)
         line = {
             "metric": "md_steps_per_s", "value": steps_per_s, "unit": "steps/s", "n_gpus": world,
             "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": 1e3 * dev_s / args.steps,
             "ms_per_step_stats": {"median": statistics.median(per_step_ms), "min": per_step_ms[0], "max": per_step_ms[-1]},
-            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
-            "config": workload_config(args.config, world),
+            "higher_is_better": True, "scaling": "strong" if sharded else "weak", "vs_baseline": None, "dtype": "f32",
+            "data": "synthetic", "config": workload_config(args.config, world, sharded),
             "pair_interactions_per_s": {"unordered": 0.5 * pairs * steps_per_s, "ordered": pairs * steps_per_s,
                                         "ordered_pairs_per_step": pairs},
             # K1 and K3 move 76 and 192 algorithmic bytes per particle and step; they are
@@ -364,14 +370,14 @@ def run_ours(args, rank, world, local_rank):
                 "frac_at_observed_clock": (achieved / fp32_peak) * sm_max_mhz / clocks["sm_mhz"]
                 if clocks and clocks.get("sm_mhz") else None,
             },
-            "e2e": {"value": aggregate_rate(world, e2e_steps, e2e_s), "unit": "steps/s", "h2d_bytes_per_step": 72 * N,
+            "e2e": {"value": aggregate_rate(1 if sharded else world, e2e_steps, e2e_s), "unit": "steps/s", "h2d_bytes_per_step": 72 * N,
                     "d2h_bytes_per_step": 72 * N, "steps": e2e_steps,
                     "what": "independent one-step requests through the C ABI, every step: pasta_set_state_host_async(x,v,F) "
                             "[pinned host -> device] + pasta_step(1) + pasta_get_state_host_async(x,v,F) [device -> pinned "
                             "host]; the library pipelines the copies on two side streams (double-buffered staging); "
                             "pasta_host_sync at the end, inside the timed region",
                     "serial_feedback_chain": {
-                        "value": aggregate_rate(world, e2e_steps, e2e_serial_s), "unit": "steps/s",
+                        "value": aggregate_rate(1 if sharded else world, e2e_steps, e2e_serial_s), "unit": "steps/s",
                         "what": "pasta_set_state_host + pasta_step(1) + pasta_get_state_host with the result fed back as the "
                                 "next input (blocking; copies and compute strictly serial)"}},
             "gpu_launches": launches, "wall_s": t_wall, "clocks": clocks,
@@ -450,6 +456,8 @@ def main():
     ap.add_argument("--sweep", type=int, default=0, choices=[0, 3, 5],
                     help="run the whole decompression of config 3 or 5 and report steps/s against density")
     ap.add_argument("--sweep-chunk", type=int, default=1000)
+    ap.add_argument("--shard", action="store_true", help="with --gpus N > 1: one simulation sharded by targets over the N "
+                    "GPUs (strong scaling) instead of N independent replicas")
     ap.add_argument("--seed", type=int, default=1, help="seed of the synthetic start (rank r uses seed + r)")
     ap.add_argument("--params", default="", help="comma-separated pasta_params overrides: a second reported mode, "
                     "e.g. r_nuc=11.5 (the paper's range split) or skip_exact_zeros=0")

@@ -245,6 +245,32 @@ int64_t pasta_launch_count(const pasta_sim* sim);
  * (pasta_launch_count counts the kernels inside a replayed step as launched). */
 int64_t pasta_graph_replays(const pasta_sim* sim);
 
+/*
+ * Target-sharded evaluation on several GPUs (the paper's P x Q force
+ * decomposition with Q = 1).  Every rank holds the WHOLE state (positions, velocities, species) and keeps it
+ * bit-identical; of every force evaluation it computes only the targets of its own stretch of the cell-sorted order
+ * (the sorted slots [bounds[rank], bounds[rank+1]) of pasta_shard_bounds: contiguous in space along the sort, balanced
+ * by the estimated pair work of the two species), leaves zeros elsewhere, and the ranks' partial F (3 N doubles) and e
+ * (N doubles) are then summed in place by `allreduce` -- the paper's MPI_Allreduce of the forces; every
+ * particle's force is complete on exactly one rank, so the sum is exact and the result is bit-identical to the
+ * one-GPU evaluation.  Cell list and integration are replicated (they cost a few % of a step).
+ *   allreduce(dev_ptr, n, user): sum the n doubles at dev_ptr over all ranks, in place, ordered with the simulation's
+ *   stream (the Python binding issues torch.distributed.all_reduce on it); returns 0 on success.
+ * world == 1 switches sharding off.  EINVAL: rank outside [0, world), world < 1, allreduce NULL with world > 1.
+ */
+typedef int (*pasta_allreduce_fn)(void* dev_ptr, int64_t n_doubles, void* user);
+int pasta_set_shard(pasta_sim* sim, int32_t rank, int32_t world, pasta_allreduce_fn allreduce, void* user);
+/*
+ * The partition pasta_set_shard uses (host arithmetic only; no GPU needed): bounds_host[0..world] with bounds[0] = 0,
+ * bounds[world] = N, non-decreasing.  Sorted slots [0, Np) are protons, [Np, N) neutrons; a proton target costs
+ * cost_p and a neutron target cost_n (any positive units), and every rank gets the same total cost up to one target.
+ * EINVAL: N <= 0, Np outside [0, N], world < 1, a cost <= 0, bounds_host NULL.
+ */
+int pasta_shard_bounds(int64_t N, int64_t Np, double cost_p, double cost_n, int32_t world, int64_t* bounds_host);
+/* The costs pasta_set_shard feeds it: streamed candidates times their evaluation cost at uniform density --
+ * out2_host = {cost of a proton target, cost of a neutron target} for the simulation's parameters (host only). */
+int pasta_shard_costs(const pasta_sim* sim, double* out2_host);
+
 const char* pasta_last_error(void);
 const char* pasta_version(void);
 

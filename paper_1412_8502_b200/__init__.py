@@ -4,4 +4,4 @@
 workloads.  Importing this package loads neither torch nor the CUDA library.
 """
 from . import inputs  # noqa: F401
-from .binding import Env, Params, PastaError, Sim, default_params, library_path, load  # noqa: F401
+from .binding import Env, Params, PastaError, Sim, default_params, library_path, load, shard_bounds  # noqa: F401

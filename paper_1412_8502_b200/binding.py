@@ -35,6 +35,7 @@ class Params(C.Structure):
 
 _ALLOC_FN = C.CFUNCTYPE(C.c_void_p, C.c_size_t, C.c_void_p)
 _FREE_FN = C.CFUNCTYPE(None, C.c_void_p, C.c_void_p)
+_ALLREDUCE_FN = C.CFUNCTYPE(C.c_int, C.c_void_p, C.c_int64, C.c_void_p)
 
 
 class Env(C.Structure):
@@ -79,6 +80,9 @@ SIGNATURES = {
     "pasta_get_timing": (C.c_int, [C.c_void_p, C.POINTER(C.c_double), C.POINTER(C.c_int64)]),
     "pasta_launch_count": (C.c_int64, [C.c_void_p]),
     "pasta_graph_replays": (C.c_int64, [C.c_void_p]),
+    "pasta_set_shard": (C.c_int, [C.c_void_p, C.c_int32, C.c_int32, _ALLREDUCE_FN, C.c_void_p]),
+    "pasta_shard_bounds": (C.c_int, [C.c_int64, C.c_int64, C.c_double, C.c_double, C.c_int32, C.POINTER(C.c_int64)]),
+    "pasta_shard_costs": (C.c_int, [C.c_void_p, C.POINTER(C.c_double)]),
     "pasta_last_error": (C.c_char_p, []),
     "pasta_version": (C.c_char_p, []),
 }
@@ -105,6 +109,13 @@ def load():
 def _check(rc):
     if rc != 0:
         raise PastaError(rc, load().pasta_last_error().decode())
+
+
+def shard_bounds(N, Np, cost_p, cost_n, world):
+    """pasta_shard_bounds: the sorted-slot stretch of every rank (host arithmetic only, no GPU needed)."""
+    out = (C.c_int64 * (int(world) + 1))()
+    _check(load().pasta_shard_bounds(int(N), int(Np), float(cost_p), float(cost_n), int(world), out))
+    return [int(b) for b in out]
 
 
 def default_params(**overrides):
@@ -381,3 +392,44 @@ class Sim:
 
     def graph_replays(self):
         return int(self.lib.pasta_graph_replays(self._h))
+
+    # -- target sharding over several GPUs (pasta_set_shard) -------------------------------------------
+    def _f64_view(self, ptr, n):
+        """The n doubles at device address ptr as a torch tensor (ptr lies inside one of the library's buffers,
+        which are torch tensors handed out through pasta_env.alloc)."""
+        for base, t in self._pool.items():
+            if base <= ptr and ptr + 8 * n <= base + t.numel():
+                return t[ptr - base: ptr - base + 8 * n].view(self._torch.float64)
+        raise ValueError("pasta: allreduce on a pointer that is not inside a library buffer")
+
+    def set_shard(self, rank, world, group=None, allreduce=None):
+        """pasta_set_shard: this process evaluates the targets of stretch `rank` of `world` of the cell-sorted order;
+        the partial forces/energies are summed over the ranks with torch.distributed.all_reduce on `group` (NCCL over
+        NVLink on a multi-GPU node), ordered with the simulation's stream.  `allreduce` (a callable taking the tensor)
+        replaces the collective -- the tests use it to play the ranks one after another on a single GPU."""
+        torch = self._torch
+
+        def _cb(ptr, n, _user):
+            try:
+                t = self._f64_view(int(ptr), int(n))
+                with torch.cuda.stream(self.stream):
+                    if allreduce is not None:
+                        allreduce(t)
+                    else:
+                        import torch.distributed as dist
+
+                        dist.all_reduce(t, op=dist.ReduceOp.SUM, group=group)
+                return 0
+            except Exception:  # no exception crosses the ABI
+                import traceback
+
+                traceback.print_exc()
+                return 1
+
+        self._shard_cb = _ALLREDUCE_FN(_cb) if int(world) > 1 else _ALLREDUCE_FN()
+        _check(self.lib.pasta_set_shard(self._h, int(rank), int(world), self._shard_cb, None))
+
+    def shard_costs(self):
+        out = (C.c_double * 2)()
+        _check(self.lib.pasta_shard_costs(self._h, out))
+        return float(out[0]), float(out[1])

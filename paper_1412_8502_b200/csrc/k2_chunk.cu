@@ -53,6 +53,7 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) k2_chunk_kernel(const ChunkA
   const unsigned active = __ballot_sync(0xffffffffu, slot >= 0);
   if (active == 0) return;  // empty primary entry
   const int slot0 = __shfl_sync(0xffffffffu, slot, 0);
+  if (slot0 < A.slot_lo || slot0 >= A.slot_hi) return;  // another rank's targets (pasta_set_shard)
   const bool chunk_p = slot0 < A.Np;
   const int st_sp = chunk_p ? 0 : 1;
   const SpeciesGrid& gt = A.g[st_sp];
@@ -90,6 +91,8 @@ int k2_chunk_forces(Sim* s, bool with_energy, bool stats) {
   A.chunk_tab = s->chunk_tab.as<int32_t>();
   A.counts = s->counters.as<int32_t>() + 2 * 24;
   A.nprim = (int32_t)s->chunk_nprim;
+  A.slot_lo = s->shard.slot_lo;
+  A.slot_hi = s->shard.slot_hi;
   A.merged = s->grid_sp[0].ncell == s->grid_sp[1].ncell && s->grid_sp[0].ncx == s->grid_sp[1].ncx ? 1 : 0;
   for (int sp = 0; sp < 2; ++sp) {
     const Grid& g = s->grid_sp[sp];

@@ -51,6 +51,7 @@ struct ChunkArgs {
   const int32_t* chunk_tab;  // [chunk][8] sorted slots of the chunk's targets, -1 = none (k1_cells.cu)
   const int32_t* counts;     // [0] number of chunks in the overflow region
   int32_t nprim;             // primary entries (some of them empty)
+  int32_t slot_lo, slot_hi;  // target sharding: only chunks whose first target's slot lies in [slot_lo, slot_hi) are evaluated
   int32_t merged;            // the two species' grids are identical: neutron chunks take both in one pass
   SpeciesGrid g[2];
   float rcS;     // sigma * r_c

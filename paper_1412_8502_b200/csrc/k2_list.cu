@@ -37,6 +37,7 @@ __device__ __forceinline__ float rsqrt_ftz(float x) {
 
 struct TListArgs {
   int32_t N, Np;
+  int32_t slot_lo, slot_hi; // target sharding: the force kernel evaluates the targets in sorted slots [slot_lo, slot_hi)
   int32_t ncell, ncx;       // ONE grid geometry for both species (list mode)
   int32_t base[2];          // first bin of each species
   float wS, wxS;            // sigma * cell width (y, z) and (x)
@@ -293,10 +294,10 @@ __device__ __forceinline__ void run_tlist(const TListArgs& A, const PairConsts& 
 
 template <bool CUT, bool ENERGY>
 __global__ void __launch_bounds__(256) k2_tlist_kernel(const TListArgs A, const PairConsts c) {
-  const int gt = blockIdx.x * (blockDim.x / GL) + (threadIdx.x / GL);
+  const int gt = A.slot_lo + blockIdx.x * (blockDim.x / GL) + (threadIdx.x / GL);
   const int h = threadIdx.x & (GL - 1);
-  const bool valid = gt < A.N;
-  const int t = valid ? gt : A.N - 1;
+  const bool valid = gt < A.slot_hi;
+  const int t = valid ? gt : A.slot_hi - 1;
   const float4 tq = __ldg(A.pos4 + t);
   const bool tp = t < A.Np;
   int4 tl = __ldg(A.tl + t);
@@ -335,6 +336,8 @@ static int tlist_args(Sim* s, TListArgs* out, double halo) {
   }
   A.N = (int32_t)s->N;
   A.Np = (int32_t)s->Np;
+  A.slot_lo = s->shard.slot_lo < 0 ? 0 : s->shard.slot_lo;
+  A.slot_hi = s->shard.slot_hi > A.N ? A.N : s->shard.slot_hi;
   A.ncell = g.ncell;
   A.ncx = g.ncx;
   A.base[0] = (int32_t)s->bin_base[0];
@@ -401,7 +404,8 @@ int k2_list_forces(Sim* s, bool with_energy) {
   const bool cut = (double)c.rn2s < 127.0;  // the nuclear cut-off lies inside the FP32 underflow distance
   TListArgs A;
   PASTA_TRY(tlist_args(s, &A, 0.0));
-  const int grid = grid_for(s->N * GL, 256);
+  if (A.slot_hi <= A.slot_lo) return PASTA_OK;  // this rank owns no target (pasta_set_shard)
+  const int grid = grid_for((int64_t)(A.slot_hi - A.slot_lo) * GL, 256);
   if (with_energy) {
     if (cut) k2_tlist_kernel<true, true><<<grid, 256, 0, s->stream>>>(A, c);
     else k2_tlist_kernel<false, true><<<grid, 256, 0, s->stream>>>(A, c);

@@ -114,12 +114,39 @@ struct Timer {
 // built with a halo and reused; every evaluation first refreshes the sorted coordinates and reads back the largest
 // displacement D since the build, and rebuilds when a pair could have entered the reach unseen:
 //   own + source displacement 2 D > halo  (less reach (L0/L - 1) if the box has shrunk since).
+// The sorted slots whose targets this rank evaluates (pasta_set_shard): the whole range on one GPU.
+static int shard_window(Sim* s) {
+  s->shard.slot_lo = 0;
+  s->shard.slot_hi = 0x7fffffff;
+  if (s->shard.world <= 1) return PASTA_OK;
+  std::vector<int64_t> b((size_t)s->shard.world + 1);
+  double cost[2];
+  PASTA_TRY(pasta_shard_costs(reinterpret_cast<const pasta_sim*>(s), cost));
+  PASTA_TRY(pasta_shard_bounds(s->N, s->Np, cost[0], cost[1], s->shard.world, b.data()));
+  s->shard.slot_lo = (int32_t)b[(size_t)s->shard.rank];
+  s->shard.slot_hi = (int32_t)b[(size_t)s->shard.rank + 1];
+  return PASTA_OK;
+}
+
 static int evaluate_forces_tail(Sim* s, bool with_energy) {
   s->n_force_evals += 1;
+  const bool sharded = s->shard.world > 1;
+  PASTA_TRY(shard_window(s));
   {
     Timer t(s, 1);
+    if (sharded) {  // the other ranks' targets stay zero: the sum over ranks then completes every particle exactly
+      PASTA_CUDA_OK(cudaMemsetAsync(s->F.ptr, 0, 24 * (size_t)s->N, s->stream));
+      if (with_energy) PASTA_CUDA_OK(cudaMemsetAsync(s->e.ptr, 0, 8 * (size_t)s->N, s->stream));
+    }
     if (s->list.valid) PASTA_TRY(k2_list_forces(s, with_energy));
     else PASTA_TRY(k2_forces(s, with_energy));
+    if (sharded) {
+      if (s->shard.allreduce(s->F.ptr, 3 * s->N, s->shard.user) != 0 ||
+          (with_energy && s->shard.allreduce(s->e.ptr, s->N, s->shard.user) != 0)) {
+        set_error("pasta_set_shard: the allreduce callback failed");
+        return PASTA_ECUDA;
+      }
+    }
   }
   if (s->timing) s->n_timed += 1;
   s->forces_valid = true;
@@ -206,6 +233,7 @@ static void graphs_destroy(Sim* s) {
 static int step_once(Sim* s, double dt, double sc, double L_wrap, bool energy, bool rescale) {
   const bool eligible = s->tune.graphs != 0 && sc == 1.0 && !(s->prm.xi_dot > 0.0) && !s->timing && !s->list.valid &&
                         s->tune.force_variant == 0 && s->forces_valid && !list_mode_wanted(s) && s->sort_kind == 0 &&
+                        s->shard.world <= 1 &&
                         s->bins_zeroed >= s->grid_sp[0].nc3 + s->grid_sp[1].nc3 + 1;
   if (!eligible) {
     s->graph.warm = 0;
@@ -916,6 +944,62 @@ int pasta_get_timing(pasta_sim* sim, double* ms3_host, int64_t* n_force_evals_ho
 int64_t pasta_launch_count(const pasta_sim* sim) {
   const Sim* s = reinterpret_cast<const Sim*>(sim);
   return s ? s->launches : 0;
+}
+
+int pasta_set_shard(pasta_sim* sim, int32_t rank, int32_t world, pasta_allreduce_fn allreduce, void* user) {
+  Sim* s = reinterpret_cast<Sim*>(sim);
+  PASTA_TRY(check_sim(s));
+  if (world < 1 || rank < 0 || rank >= world || (world > 1 && !allreduce)) {
+    set_error("pasta_set_shard: need world >= 1, 0 <= rank < world and an allreduce callback when world > 1");
+    return PASTA_EINVAL;
+  }
+  s->shard.rank = rank;
+  s->shard.world = world;
+  s->shard.allreduce = allreduce;
+  s->shard.user = user;
+  s->forces_valid = false;  // whatever F holds was computed under the old partition
+  s->energies_valid = false;
+  return PASTA_OK;
+}
+
+int pasta_shard_bounds(int64_t N, int64_t Np, double cost_p, double cost_n, int32_t world, int64_t* bounds_host) {
+  if (N <= 0 || Np < 0 || Np > N || world < 1 || !(cost_p > 0.0) || !(cost_n > 0.0) || !bounds_host) {
+    set_error("pasta_shard_bounds: need N > 0, 0 <= Np <= N, world >= 1, positive costs and a bounds array");
+    return PASTA_EINVAL;
+  }
+  // cumulative cost of the sorted slots [0, t): protons first, then neutrons; rank r starts at the first slot whose
+  // cumulative cost reaches r / world of the total
+  const double total = cost_p * (double)Np + cost_n * (double)(N - Np);
+  bounds_host[0] = 0;
+  for (int32_t r = 1; r < world; ++r) {
+    const double want = total * (double)r / (double)world;
+    const double in_p = cost_p * (double)Np;
+    double t = want <= in_p ? want / cost_p : (double)Np + (want - in_p) / cost_n;
+    int64_t b = (int64_t)floor(t + 0.5);
+    b = b < bounds_host[r - 1] ? bounds_host[r - 1] : (b > N ? N : b);
+    bounds_host[r] = b;
+  }
+  bounds_host[world] = N;
+  return PASTA_OK;
+}
+
+int pasta_shard_costs(const pasta_sim* sim, double* out2_host) {
+  const Sim* s = reinterpret_cast<const Sim*>(sim);
+  PASTA_TRY(check_sim(s));
+  if (!out2_host) {
+    set_error("out2_host is NULL");
+    return PASTA_EINVAL;
+  }
+  // candidates within the reach of a pass (a sphere's worth at uniform density) times the cost of evaluating one:
+  // a proton-proton candidate (screened Coulomb: 21 packed FP32 + 6 MUFU) costs about 1.64 np/nn candidates (13 + 2)
+  const double sigma = sqrt(1.4426950408889634074 / (2.0 * s->prm.Lambda));
+  double r_n = s->prm.r_nuc > 0.0 ? s->prm.r_nuc : s->prm.r_c;
+  if (s->prm.skip_exact_zeros && sigma * r_n > 11.2472) r_n = 11.2472 / sigma;
+  const double vp = s->prm.r_c * s->prm.r_c * s->prm.r_c, vn = r_n * r_n * r_n;
+  const double np = (double)s->Np, nn = (double)(s->N - s->Np);
+  out2_host[0] = 1.64 * np * vp + nn * vn + 1.0;
+  out2_host[1] = (np + nn) * vn + 1.0;
+  return PASTA_OK;
 }
 
 int64_t pasta_graph_replays(const pasta_sim* sim) {

@@ -258,6 +258,13 @@ struct Sim {
     cudaStream_t cap = nullptr;    // capture happens on a stream of our own (the caller's may be the legacy default stream)
     int warm = 0;                  // eligible steps enqueued kernel by kernel since the last change (buffers settle)
   } graph;
+  // target sharding over several GPUs (pasta_set_shard): this rank evaluates the targets in sorted slots [slot_lo, slot_hi)
+  struct Shard {
+    int32_t rank = 0, world = 1;
+    pasta_allreduce_fn allreduce = nullptr;
+    void* user = nullptr;
+    int32_t slot_lo = 0, slot_hi = 0x7fffffff;
+  } shard;
   int sort_kind = -1;     // what the sorted arrays and grid_sp describe: 0 chunk-path grids, 1 uniform grid, 2 list grid, -1 nothing
   int64_t state_gen = 0;  // bumped whenever a device buffer moves or the particle set changes: captured graphs are stale
 
