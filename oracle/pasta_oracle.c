@@ -33,6 +33,11 @@ typedef struct orc_params {
   double r_nuc;           /* the paper's own range split: the nuclear (Gaussian) terms are "assumed
                              to be zero and not computed" beyond r_nuc = 11.5 fm, independently of the Coulomb
                              term.  <= 0 (default): no separate nuclear cut-off, every term lives inside r_c (D1) */
+  double coul_nocut;      /* != 0: the paper's own Coulomb sum ("we do not use a cutoff radius for the
+                             Coulomb potential ... each proton interacts with the nearest periodic image of every
+                             other proton"): every proton pair interacts through its nearest image whatever the
+                             distance (a cube of side L around the target, not a sphere); needs r_nuc > 0, which then
+                             is the only cut-off of the nuclear terms.  0 (default): Coulomb lives inside r_c (D1) */
 } orc_params;
 
 int orc_num_threads(void) {
@@ -109,9 +114,9 @@ void orc_forces(int64_t N, const double* x, const uint8_t* is_p, double L, const
       double dy = nearest_image(x[3 * i + 1] - x[3 * j + 1], L);
       double dz = nearest_image(x[3 * i + 2] - x[3 * j + 2], L);
       double r2 = dx * dx + dy * dy + dz * dz;
-      if (r2 < rc2) {
+      if (r2 < rc2 || (p->coul_nocut != 0.0 && is_p[i] && is_p[j])) {
         double V, g;
-        pair_terms(p, r2, is_p[i], is_p[j], &V, &g);
+        pair_terms(p, r2, is_p[i], is_p[j], &V, &g); /* beyond r_c >= r_nuc only the Coulomb term is left */
         fx += g * dx;
         fy += g * dy;
         fz += g * dz;

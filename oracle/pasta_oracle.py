@@ -13,7 +13,7 @@ _lib = None
 
 
 class _CParams(C.Structure):
-    _fields_ = [(n, C.c_double) for n in ("a", "b", "c", "Lambda", "alpha", "lambda_", "r_c", "mass", "r_nuc")]
+    _fields_ = [(n, C.c_double) for n in ("a", "b", "c", "Lambda", "alpha", "lambda_", "r_c", "mass", "r_nuc", "coul_nocut")]
 
 
 @dataclass
@@ -29,9 +29,12 @@ class Params:
     r_c: float = 20.0
     mass: float = 939.0
     r_nuc: float = 0.0  # > 0: the paper's separate nuclear cut-off (11.5 fm); 0: none (reading D1)
+    coul_nocut: float = 0.0  # != 0: Coulomb between every proton pair at the nearest image, no radial cut-off
 
     def _c(self):
-        return _CParams(self.a, self.b, self.c, self.Lambda, self.alpha, self.lambda_, self.r_c, self.mass, self.r_nuc)
+        if self.coul_nocut and not self.r_nuc > 0.0:
+            raise ValueError("coul_nocut needs r_nuc > 0: without r_c the nuclear terms have no other cut-off (PAPER.md:98)")
+        return _CParams(self.a, self.b, self.c, self.Lambda, self.alpha, self.lambda_, self.r_c, self.mass, self.r_nuc, self.coul_nocut)
 
 
 def build(force=False):

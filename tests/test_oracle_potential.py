@@ -295,3 +295,53 @@ def test_range_split_of_the_paper(orc):
     # count: it is compared to a few ulp of itself (1 ulp of 2.5e4 MeV is 3.6e-12), not to an absolute 1e-16.
     assert np.abs(Ff - Fs).max() < 1e-19 and np.abs(ef - es).max() < 1e-19
     assert abs(pef - pes) <= 4 * np.spacing(abs(pef)) and abs(ef.sum() - es.sum()) < 1e-16
+
+
+def test_coulomb_without_cutoff_nearest_image_cube(orc):
+    """"we do not use a cutoff radius for the Coulomb potential ... each proton interacts with the
+    nearest periodic image of every other proton" while the nuclear terms stop at 11.5 fm.  Pins of the oracle's
+    coul_nocut switch: (i) a proton pair beyond r_c feels exactly the Yukawa term, repulsive, along the nearest image;
+    (ii) past L/2 along an axis the image flips; (iii) the interaction region is the CUBE of side L, not the sphere
+    of radius L/2; (iv) np and nn pairs beyond r_nuc feel nothing; (v) on a random system the switch adds exactly the
+    proton pairs beyond r_c, summed here independently with numpy; total force stays zero."""
+    L = 60.0
+    on = orc.Params(r_c=20.0, r_nuc=11.5, coul_nocut=1.0)
+    off = orc.Params(r_c=20.0, r_nuc=11.5)
+    yuk = lambda r: 1.44 * math.exp(-r / 10.0) / r
+    pp = np.array([1, 1], dtype=np.uint8)
+
+    def two(d, is_p, prm):
+        x = np.array([[5.0, 5.0, 5.0], [5.0 + d[0], 5.0 + d[1], 5.0 + d[2]]])
+        F, e, pe, _ = orc.forces(orc.wrap(x, L), is_p, L, prm)
+        return F, pe
+
+    F, pe = two((25.0, 0, 0), pp, on)                       # (i) beyond r_c, inside L/2
+    assert pe == pytest.approx(yuk(25.0), rel=1e-14)
+    assert F[0] == pytest.approx([-yuk(25.0) * (1 / 25.0 + 0.1), 0, 0], rel=1e-13, abs=1e-18) and np.allclose(F[0], -F[1], rtol=0, atol=1e-18)
+    assert two((25.0, 0, 0), pp, off)[1] == 0.0
+    F, pe = two((40.0, 0, 0), pp, on)                       # (ii) nearest image is 20 fm away on the other side
+    assert pe == pytest.approx(yuk(20.0), rel=1e-14) and F[0, 0] == pytest.approx(+yuk(20.0) * (1 / 20.0 + 0.1), rel=1e-13)
+    F, pe = two((25.0, 25.0, 25.0), pp, on)                 # (iii) r = 43.3 fm > L/2 = 30 fm, every component < L/2
+    r = 25.0 * math.sqrt(3.0)
+    assert pe == pytest.approx(yuk(r), rel=1e-14) and np.allclose(F[0], -yuk(r) * (1 / r + 0.1) / r * 25.0, rtol=1e-13)
+    for is_p in (np.array([1, 0], dtype=np.uint8), np.array([0, 0], dtype=np.uint8)):   # (iv)
+        F, pe = two((12.0, 0, 0), is_p, on)
+        assert pe == 0.0 and not F.any()
+    with pytest.raises(ValueError):
+        orc.forces(np.zeros((2, 3)), pp, L, orc.Params(r_c=20.0, coul_nocut=1.0))
+    # (v) random system: config-1 density, wider box so that L/2 > r_c leaves a shell and corners
+    x, v, is_p, Lb = inputs.uniform_state(3000, 0.3, 0.02, 1.0, seed=8)
+    Fa, ea, pea, _ = orc.forces(x, is_p, Lb, on)
+    Fb, eb, peb, _ = orc.forces(x, is_p, Lb, off)
+    xp = x[is_p == 1]
+    d = xp[:, None, :] - xp[None, :, :]
+    d -= Lb * np.round(d / Lb)
+    rr = np.sqrt((d ** 2).sum(-1))
+    far = rr >= 20.0
+    np.fill_diagonal(far, False)
+    extra = 0.5 * (1.44 * np.exp(-rr[far] / 10.0) / rr[far]).sum()
+    assert far.sum() > 1e5 and pea - peb == pytest.approx(extra, rel=1e-10)
+    gfar = np.where(far, 1.44 * np.exp(-rr / 10.0) / np.where(rr > 0, rr, 1.0) * (1.0 / np.where(rr > 0, rr, 1.0) + 0.1) / np.where(rr > 0, rr, 1.0), 0.0)
+    assert np.allclose((Fa - Fb)[is_p == 1], (gfar[:, :, None] * d).sum(1), rtol=1e-9, atol=1e-12)
+    assert not (Fa - Fb)[is_p == 0].any()
+    assert np.abs(Fa.sum(0)).max() <= 1e-10 * np.abs(Fa).sum()
