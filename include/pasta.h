@@ -72,6 +72,13 @@ typedef struct pasta_params {
                                   the box side becomes L0 (1 + xi_dot dt n), n = steps since create / set_state / expand and
                                   L0 the side at that moment; positions and velocities are NOT scaled.  Needs
                                   scale_per_step == 1 and a constant dt.  0 (default): off */
+  int32_t coulomb_all_pairs;   /* 1: the Coulomb half of the paper's range split ("we do not use a cutoff radius
+                                  for the Coulomb potential ... each proton interacts with the nearest periodic image of
+                                  every other proton"): the screened Coulomb term is summed over ALL proton pairs at their
+                                  nearest image (a cube of side L, no radial cut-off; N_p^2 pair terms by a kernel of its
+                                  own) and the nuclear terms stop at r_nuc, which must be set; r_c then only sizes the
+                                  cell list.  0 (default): the Coulomb term lives inside r_c like every other (D1) */
+  int32_t reserved1;
 } pasta_params;
 
 /* Device environment: where internal memory and the stream come from. */

@@ -30,6 +30,7 @@ class Params(C.Structure):
         ("thermostat_interval", C.c_int32), ("cell_subdiv", C.c_int32), ("energy_every_step", C.c_int32),
         ("skip_exact_zeros", C.c_int32), ("list_reuse", C.c_int32),
         ("list_halo", C.c_double), ("r_nuc", C.c_double), ("xi_dot", C.c_double),
+        ("coulomb_all_pairs", C.c_int32), ("reserved1", C.c_int32),
     ]
 
 

@@ -91,6 +91,7 @@ int k2_chunk_forces(Sim* s, bool with_energy, bool stats) {
   A.chunk_tab = s->chunk_tab.as<int32_t>();
   A.counts = s->counters.as<int32_t>() + 2 * 24;
   A.nprim = (int32_t)s->chunk_nprim;
+  A.no_coul = s->prm.coulomb_all_pairs ? 1 : 0;
   A.slot_lo = s->shard.slot_lo;
   A.slot_hi = s->shard.slot_hi;
   A.merged = s->grid_sp[0].ncell == s->grid_sp[1].ncell && s->grid_sp[0].ncx == s->grid_sp[1].ncx ? 1 : 0;

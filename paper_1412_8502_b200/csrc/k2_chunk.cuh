@@ -52,6 +52,7 @@ struct ChunkArgs {
   const int32_t* counts;     // [0] number of chunks in the overflow region
   int32_t nprim;             // primary entries (some of them empty)
   int32_t slot_lo, slot_hi;  // target sharding: only chunks whose first target's slot lies in [slot_lo, slot_hi) are evaluated
+  int32_t no_coul;           // coulomb_all_pairs: the Coulomb term is summed elsewhere (k2_coulomb.cu); nuclear terms only
   int32_t merged;            // the two species' grids are identical: neutron chunks take both in one pass
   SpeciesGrid g[2];
   float rcS;     // sigma * r_c
@@ -429,7 +430,7 @@ __device__ __forceinline__ void chunk_passes(const ChunkArgs& A, const PairConst
       k.gB = c.gB_unlike;
       k.B = c.B_unlike;
       source_pass<false, CUT, ENERGY, STATS, true>(A, c, sh, lane, gs, rx, ry, rz, b, t, acc, k, st);
-    } else if (sp == 0 && chunk_p) {
+    } else if (sp == 0 && chunk_p && A.no_coul == 0) {
       source_pass<true, CUT, ENERGY, STATS, false>(A, c, sh, lane, gs, rx, ry, rz, b, t, acc, k, st);
     } else {
       source_pass<false, CUT, ENERGY, STATS, false>(A, c, sh, lane, gs, rx, ry, rz, b, t, acc, k, st);

@@ -37,6 +37,7 @@ __device__ __forceinline__ float rsqrt_ftz(float x) {
 
 struct TListArgs {
   int32_t N, Np;
+  int32_t no_coul;          // coulomb_all_pairs: the Coulomb term is summed elsewhere (k2_coulomb.cu)
   int32_t slot_lo, slot_hi; // target sharding: the force kernel evaluates the targets in sorted slots [slot_lo, slot_hi)
   int32_t ncell, ncx;       // ONE grid geometry for both species (list mode)
   int32_t base[2];          // first bin of each species
@@ -304,7 +305,7 @@ __global__ void __launch_bounds__(256) k2_tlist_kernel(const TListArgs A, const 
   if (!valid) tl.y = tl.w = 0;
   Acc4 acc = {0.f, 0.f, 0.f, 0.f};
   // proton sources: like (+ Coulomb) for a proton target, unlike for a neutron target; then the neutron sources
-  run_tlist<CUT, ENERGY>(A, c, tq, tl.x, tl.y, h, tp, tp ? c.B_like : c.B_unlike, tp ? c.gB_like : c.gB_unlike, acc);
+  run_tlist<CUT, ENERGY>(A, c, tq, tl.x, tl.y, h, tp && A.no_coul == 0, tp ? c.B_like : c.B_unlike, tp ? c.gB_like : c.gB_unlike, acc);
   run_tlist<CUT, ENERGY>(A, c, tq, tl.z, tl.w, h, false, tp ? c.B_unlike : c.B_like, tp ? c.gB_unlike : c.gB_like, acc);
   // the 8 lanes' FP32 partial sums meet in FP64
   double fx = (double)acc.fx, fy = (double)acc.fy, fz = (double)acc.fz, ee = (double)acc.e;
@@ -336,6 +337,7 @@ static int tlist_args(Sim* s, TListArgs* out, double halo) {
   }
   A.N = (int32_t)s->N;
   A.Np = (int32_t)s->Np;
+  A.no_coul = s->prm.coulomb_all_pairs ? 1 : 0;
   A.slot_lo = s->shard.slot_lo < 0 ? 0 : s->shard.slot_lo;
   A.slot_hi = s->shard.slot_hi > A.N ? A.N : s->shard.slot_hi;
   A.ncell = g.ncell;

@@ -57,7 +57,7 @@ void buffer_release(Sim* s, Buffer* b) {
 
 static void release_all(Sim* s) {
   Buffer* bs[] = {&s->x, &s->v, &s->F, &s->e, &s->is_p, &s->cell_id, &s->bin_count, &s->bin_start, &s->scan_tmp,
-                  &s->perm, &s->perm_raw, &s->pos4, &s->cxyz, &s->partials, &s->scalars, &s->counters, &s->cl_parent, &s->cl_A,
+                  &s->perm, &s->perm_raw, &s->pos4, &s->cxyz, &s->cpos, &s->partials, &s->scalars, &s->counters, &s->cl_parent, &s->cl_A,
                   &s->cl_Z, &s->cl_cell_id, &s->cl_count, &s->cl_start, &s->cl_perm, &s->chunk_tab, &s->xref, &s->slot_of, &s->list_off,
                   &s->list_pool};
   for (Buffer* b : bs) buffer_release(s, b);
@@ -140,6 +140,7 @@ static int evaluate_forces_tail(Sim* s, bool with_energy) {
     }
     if (s->list.valid) PASTA_TRY(k2_list_forces(s, with_energy));
     else PASTA_TRY(k2_forces(s, with_energy));
+    if (s->prm.coulomb_all_pairs) PASTA_TRY(k2_coulomb_all_pairs(s, with_energy));
     if (sharded) {
       if (s->shard.allreduce(s->F.ptr, 3 * s->N, s->shard.user) != 0 ||
           (with_energy && s->shard.allreduce(s->e.ptr, s->N, s->shard.user) != 0)) {
@@ -343,6 +344,7 @@ int pasta_params_default(pasta_params* p) {
   p->list_halo = 0.0;
   p->r_nuc = 0.0;
   p->xi_dot = 0.0;
+  p->coulomb_all_pairs = 0;
   return PASTA_OK;
 }
 
@@ -359,6 +361,10 @@ static int validate_params(const pasta_params* p, double L) {
   }
   if (!(p->r_nuc >= 0.0) || p->r_nuc > p->r_c) {
     set_error("pasta_params: need 0 <= r_nuc <= r_c");
+    return PASTA_EINVAL;
+  }
+  if (p->coulomb_all_pairs != 0 && !(p->r_nuc > 0.0)) {
+    set_error("pasta_params: coulomb_all_pairs needs r_nuc > 0 (without a Coulomb cut-off r_nuc is what cuts the nuclear terms)");
     return PASTA_EINVAL;
   }
   if (!(p->xi_dot >= 0.0) || (p->xi_dot > 0.0 && p->scale_per_step != 1.0)) {

@@ -203,6 +203,7 @@ struct Sim {
   Buffer perm;        // int32[N]   sorted slot -> original index
   Buffer pos4;        // float4[N]  sorted: sigma * cell-relative position, .w = cell x index
   Buffer cxyz;        // int32[N]   sorted: packed cell coordinates (cx | cy<<10 | cz<<20)
+  Buffer cpos;        // float4[2 Np] sorted protons as box fractions x / L, hi and lo parts (k2_coulomb.cu)
 
   // reductions
   Buffer partials;    // double[>= 4096]
@@ -300,6 +301,7 @@ int k2_reference_forces(Sim* s, bool with_energy);     // variant 1: thread per 
 int k2_chunk_forces(Sim* s, bool with_energy, bool stats);  // variant 2: chunk kernel (k2_chunk.cu)
 int k2_list_build(Sim* s, double halo);                // neighbour lists of the sorted order k1_build just made (k2_list.cu)
 int k2_list_forces(Sim* s, bool with_energy);          // the pair kernel on those lists
+int k2_coulomb_all_pairs(Sim* s, bool with_energy);    // += screened Coulomb of every proton pair, nearest image (k2_coulomb.cu)
 // K3  k3_integrate.cu
 int k3_init_state(Sim* s, uint64_t seed);
 int k3_kick_drift_refresh(Sim* s, double dt, double scale, double L_wrap);  // list mode: kick, drift + the refresh of the frozen order

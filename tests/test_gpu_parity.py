@@ -792,3 +792,34 @@ def test_captured_step_equals_kernel_by_kernel(monkeypatch):
     with pasta.Sim(8192, 0.3, 0.05, 1.0, params=p, seed=11) as sim:
         sim.step(12, 2.0)
         assert sim.graph_replays() == 0
+
+
+@pytest.mark.parametrize("N,Y_P,density,path", [(30000, 0.4, 0.0125, "chunk"), (60000, 0.3, 0.03, "chunk"),
+                                                (20000, 0.2, 0.00125, "list")])
+def test_coulomb_without_cutoff_mode(orc, N, Y_P, density, path):
+    """SURVEY 8(f) rank 1, second half: the screened Coulomb term over ALL proton pairs at their nearest
+    image, no radial cut-off (k2_coulomb.cu), nuclear terms cut at r_nuc = 11.5 fm by the chunk / list kernels.  Forces,
+    per-particle energies and PE against the oracle's coul_nocut mode, same gates as the contract mode; then 5 MD steps.
+    (Boxes of >= 120 fm: the nearest-image decision is taken on FP32 box fractions, and a pair within 1e-5 fm of
+    |d| = L/2 along an axis may take the other image -- a jump of 2 F_c(L/2), 7e-6 MeV/fm at L = 120 fm; reading D26.)"""
+    x, v, is_p, L = inputs.uniform_state(N, Y_P, density, 0.5, seed=31)
+    op = orc.Params(r_c=20.0, r_nuc=11.5, coul_nocut=1.0)
+    with _sim_from_arrays(x, v, is_p, L, T=0.5, r_c=20.0, r_nuc=11.5, coulomb_all_pairs=1, thermostat_interval=0) as sim:
+        F, pe = sim.forces()
+        e = _np(sim.particle_energies())
+        st = sim.list_stats()
+        Fo, eo, peo, d = orc.forces(x, is_p, L, op)
+        _check_forces(_np(F), Fo, pe, peo)
+        assert np.abs(e - eo).max() <= 2e-6 * np.abs(eo).max()
+        # the far pairs are really there: against the radial mode the energy differs by the Coulomb tail beyond r_c
+        _, _, pe_cut, _ = orc.forces(x, is_p, L, orc.Params(r_c=20.0, r_nuc=11.5))
+        assert peo - pe_cut > 50 * PE_TOL * abs(peo)
+        sim.step(5, 2.0)
+        xg = _np(sim.get_state()[0])
+        xo = orc.step(x, v, is_p, L, op, 0.5, 0, 1.0, 2.0, 5)[0]
+        dd = xg - xo
+        dd -= L * np.round(dd / L)
+        assert np.quantile(np.linalg.norm(dd, axis=1), 0.999) <= TRAJ_TOL
+        assert (sim.list_stats()["list_builds"] < sim.list_stats()["force_evals"]) == (path == "list")
+    with pytest.raises(pasta.PastaError):
+        pasta.Sim(N, Y_P, density, 1.0, params=pasta.default_params(coulomb_all_pairs=1), seed=1)
