@@ -407,19 +407,32 @@ def run_sweep(args):
                                scale_per_step=c["scale_per_step"])
     sim = pasta.Sim(c["N"], c["Y_P"], c["density"], c["T"], params=prm, seed=1)
     pts, done = [], 0
+    sm_max_mhz, _, _ = peaks()
+    fp32_peak = SM_COUNT * FP32_LANES_PER_SM * sm_max_mhz * 1e6
+    n_brk = 10  # steps at the end of every chunk that run with the library's event brackets on (K2 time for the roofline)
     t_all0 = time.perf_counter()
     while done < c["steps"]:
         n = min(args.sweep_chunk, c["steps"] - done)
         a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         a.record()
-        sim.step(n, c["dt"])
+        sim.step(n - n_brk, c["dt"])
         b.record()
+        sim.set_timing(True)
+        sim.step(n_brk, c["dt"])
+        tm = sim.get_timing()
+        sim.set_timing(False)
         torch.cuda.synchronize()
         done += n
         L = sim.box_length()
         ke, pe = sim.energy()
-        pts.append({"step": done, "L_fm": L, "density": c["N"] / L ** 3, "steps_per_s": 1e3 * n / a.elapsed_time(b),
-                    "PE_per_nucleon": pe / c["N"], "T_kin": ke / (1.5 * c["N"])})
+        pairs, pairs_nz = sim.pair_counts()
+        k2_s = tm["force_ms"] * 1e-3 / max(1, tm["force_evals"])
+        work = 17.0 * pairs_nz + 8.0 * c["Y_P"] ** 2 * pairs  # as in the headline: only pairs with a non-zero FP32 term
+        pts.append({"step": done, "L_fm": L, "density": c["N"] / L ** 3, "steps_per_s": 1e3 * (n - n_brk) / a.elapsed_time(b),
+                    "PE_per_nucleon": pe / c["N"], "T_kin": ke / (1.5 * c["N"]),
+                    "ordered_pairs": pairs, "nonzero_pairs": pairs_nz, "k2_ms": 1e3 * k2_s,
+                    "roofline": {"bound": "alu", "frac": work / k2_s / fp32_peak, "achieved": work / k2_s / 1e9,
+                                 "peak": fp32_peak / 1e9, "unit": "G FP32 lane-instr/s, work performed"}})
     wall = time.perf_counter() - t_all0
     list_stats = sim.list_stats()
     t0 = time.perf_counter()
