@@ -578,6 +578,11 @@ void k1_refresh_args(Sim* s, RefreshArgs* out) {
   R.scratch = s->counters.as<unsigned>() + 2 * 28;  // counters[28]: {max bits, ticket}
   R.mbox = s->list.mbox_dev;
   R.seq = ++s->list.seq;
+  {
+    const double ratio = s->L / s->list.L0;
+    R.delta = s->list.halo + (ratio >= 1.0 ? 0.0 : s->prm.r_c * (1.0 - 1.0 / ratio));
+  }
+  R.gate = s->counters.as<unsigned>() + 2 * 31;  // counters[31]
 }
 
 // The host decides whether the lists survive this step: wait for the post of the refresh (a few microseconds after

@@ -37,6 +37,9 @@ __device__ __forceinline__ float rsqrt_ftz(float x) {
 
 struct TListArgs {
   int32_t N, Np;
+  const unsigned* gate;     // != NULL: evaluate only if *gate != 0 (the refresh enqueued before this kernel lets the lists live)
+  double* v;                // kick != 0: the second half kick v += kick F rides along (O2 step 4)
+  double kick;
   int32_t no_coul;          // coulomb_all_pairs: the Coulomb term is summed elsewhere (k2_coulomb.cu)
   int32_t slot_lo, slot_hi; // target sharding: the force kernel evaluates the targets in sorted slots [slot_lo, slot_hi)
   int32_t ncell, ncx;       // ONE grid geometry for both species (list mode)
@@ -295,6 +298,7 @@ __device__ __forceinline__ void run_tlist(const TListArgs& A, const PairConsts& 
 
 template <bool CUT, bool ENERGY>
 __global__ void __launch_bounds__(256) k2_tlist_kernel(const TListArgs A, const PairConsts c) {
+  if (A.gate && *A.gate == 0u) return;  // a particle has left its halo: the host rebuilds and evaluates again
   const int gt = A.slot_lo + blockIdx.x * (blockDim.x / GL) + (threadIdx.x / GL);
   const int h = threadIdx.x & (GL - 1);
   const bool valid = gt < A.slot_hi;
@@ -322,6 +326,12 @@ __global__ void __launch_bounds__(256) k2_tlist_kernel(const TListArgs A, const 
     A.F[3 * (int64_t)i + 1] = -fy;
     A.F[3 * (int64_t)i + 2] = -fz;
     if (ENERGY) A.e[i] = 0.5 * ee;
+    if (A.kick != 0.0) {  // the arithmetic of k3_kick_ke_kernel on the stored force
+      const double Fx = -fx, Fy = -fy, Fz = -fz;
+      A.v[3 * (int64_t)i + 0] = A.v[3 * (int64_t)i + 0] + A.kick * Fx;
+      A.v[3 * (int64_t)i + 1] = A.v[3 * (int64_t)i + 1] + A.kick * Fy;
+      A.v[3 * (int64_t)i + 2] = A.v[3 * (int64_t)i + 2] + A.kick * Fz;
+    }
   }
 }
 
@@ -337,6 +347,9 @@ static int tlist_args(Sim* s, TListArgs* out, double halo) {
   }
   A.N = (int32_t)s->N;
   A.Np = (int32_t)s->Np;
+  A.gate = nullptr;
+  A.v = s->v.as<double>();
+  A.kick = 0.0;
   A.no_coul = s->prm.coulomb_all_pairs ? 1 : 0;
   A.slot_lo = s->shard.slot_lo < 0 ? 0 : s->shard.slot_lo;
   A.slot_hi = s->shard.slot_hi > A.N ? A.N : s->shard.slot_hi;
@@ -401,11 +414,13 @@ int k2_list_build(Sim* s, double halo) {
   return PASTA_ESTATE;
 }
 
-int k2_list_forces(Sim* s, bool with_energy) {
+int k2_list_forces(Sim* s, bool with_energy, bool gated, double kick) {
   const PairConsts c = make_pair_consts(s->prm);
   const bool cut = (double)c.rn2s < 127.0;  // the nuclear cut-off lies inside the FP32 underflow distance
   TListArgs A;
   PASTA_TRY(tlist_args(s, &A, 0.0));
+  if (gated) A.gate = s->counters.as<unsigned>() + 2 * 31;
+  A.kick = kick;
   if (A.slot_hi <= A.slot_lo) return PASTA_OK;  // this rank owns no target (pasta_set_shard)
   const int grid = grid_for((int64_t)(A.slot_hi - A.slot_lo) * GL, 256);
   if (with_energy) {

@@ -193,7 +193,63 @@ static int evaluate_forces(Sim* s, bool with_energy) {
 
 // One MD step with s->L already set to the box the forces are evaluated in (O2: first half kick + drift, forces,
 // second half kick, rescale on every thermostat_interval-th step).
+// A step on reused neighbour lists without a round trip to the host in its critical path: the
+// kick-drift kernel refreshes the frozen order, measures the largest displacement since the build and DECIDES on the
+// device whether the lists survive (2 D <= halo); the force kernel -- with the second half kick riding along -- is
+// enqueued right behind it and returns at once if they do not.  The host reads the same decision from its mailbox
+// while the force kernel runs; only when the trigger has fired does it rebuild and evaluate again.
+static int list_step(Sim* s, double dt, double sc, double L_wrap, bool energy, bool rescale, bool* done) {
+  *done = false;
+  const double ratio = s->L / s->list.L0;
+  // what the host alone can tell: the frozen grid is still good for this box, and lists are still wanted in it
+  if (ratio > 1.05 || ratio < 0.95 || !list_mode_wanted(s) || s->shard.world > 1 || s->prm.coulomb_all_pairs) return PASTA_OK;
+  {
+    Timer t(s, 2);
+    PASTA_TRY(k3_kick_drift_refresh(s, dt, sc, L_wrap));
+    s->lin_n += 1;
+  }
+  s->clusters_valid = false;
+  *done = true;
+  const double h2 = dt / (2.0 * s->prm.mass);
+  {
+    Timer t(s, 1);
+    PASTA_TRY(k2_list_forces(s, energy, true, rescale ? 0.0 : h2));
+  }
+  double d = 0.0;
+  PASTA_TRY(k1_refresh_wait(s, &d));
+  const double delta = s->list.halo + (ratio >= 1.0 ? 0.0 : s->prm.r_c * (1.0 - 1.0 / ratio));
+  if (2.0 * d <= delta) {  // (the device took the same decision in the same arithmetic)
+    s->n_force_evals += 1;
+    if (s->timing) s->n_timed += 1;
+    s->forces_valid = true;
+    s->energies_valid = energy;
+    s->step_count += 1;
+    if (rescale) {
+      Timer t(s, 2);
+      PASTA_TRY(k3_kick_ke(s, dt, true));
+    }
+    return PASTA_OK;
+  }
+  // the gated kernel did nothing: rebuild, evaluate, kick
+  s->list.valid = false;
+  s->forces_valid = false;
+  PASTA_TRY(evaluate_forces(s, energy));
+  s->step_count += 1;
+  {
+    Timer t(s, 2);
+    PASTA_TRY(k3_kick_ke(s, dt, rescale));
+  }
+  return PASTA_OK;
+}
+
+// One MD step with s->L already set to the box the forces are evaluated in (O2: first half kick + drift, forces,
+// second half kick, rescale on every thermostat_interval-th step).
 static int step_body(Sim* s, double dt, double sc, double L_wrap, bool energy, bool rescale) {
+  if (s->list.valid) {
+    bool done = false;
+    PASTA_TRY(list_step(s, dt, sc, L_wrap, energy, rescale, &done));
+    if (done) return PASTA_OK;
+  }
   {
     Timer t(s, 2);
     // the cell histogram of the new positions rides along unless the sorted order is frozen (or about to be

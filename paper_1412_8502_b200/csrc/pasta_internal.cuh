@@ -94,6 +94,8 @@ struct RefreshArgs {
   unsigned* scratch;      // {max displacement^2 (float bits), blocks finished}; zero between launches
   unsigned long long* mbox;
   unsigned seq;
+  double delta;           // the lists survive iff 2 * displacement <= delta (halo, less what a shrunken box took of it)
+  unsigned* gate;         // device word: 1 = the lists survive this step (read by the force kernel enqueued behind), 0 = not
 };
 // pos4[slot] = sigma * (x - centre of the slot's frozen cell), nearest image -- bit for bit k1_gather_kernel's value
 // while the particle is inside its cell; returns its squared displacement since the build, measured in co-moving
@@ -132,6 +134,9 @@ __device__ __forceinline__ void refresh_post(const RefreshArgs& R, float d2) {
     if (atomicAdd(R.scratch + 1, 1u) == gridDim.x - 1) {
       const unsigned m = atomicExch(R.scratch, 0u);
       R.scratch[1] = 0u;
+      // the trigger, decided here in the host's arithmetic, so that the force kernel already enqueued behind this one
+      // runs (or returns at once) without a round trip to the host
+      *R.gate = 2.0 * sqrt((double)__uint_as_float(m)) <= R.delta ? 1u : 0u;
       *reinterpret_cast<volatile unsigned long long*>(R.mbox) = ((unsigned long long)R.seq << 32) | m;
       __threadfence_system();
     }
@@ -300,7 +305,8 @@ int k2_pair_count(Sim* s, int64_t* ordered_pairs_host, int64_t* nonzero_pairs_ho
 int k2_reference_forces(Sim* s, bool with_energy);     // variant 1: thread per target (k2_force.cu)
 int k2_chunk_forces(Sim* s, bool with_energy, bool stats);  // variant 2: chunk kernel (k2_chunk.cu)
 int k2_list_build(Sim* s, double halo);                // neighbour lists of the sorted order k1_build just made (k2_list.cu)
-int k2_list_forces(Sim* s, bool with_energy);          // the pair kernel on those lists
+int k2_list_forces(Sim* s, bool with_energy, bool gated = false, double kick = 0.0);  // the pair kernel on those lists; gated:
+                                                       // only if the refresh just enqueued lets the lists live; kick: v += kick F
 int k2_coulomb_all_pairs(Sim* s, bool with_energy);    // += screened Coulomb of every proton pair, nearest image (k2_coulomb.cu)
 // K3  k3_integrate.cu
 int k3_init_state(Sim* s, uint64_t seed);
