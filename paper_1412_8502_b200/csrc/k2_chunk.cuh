@@ -37,6 +37,12 @@ __device__ __forceinline__ float rsqrt_approx(float x) {
   return y;
 }
 __device__ __forceinline__ float2 dup(float a) { return make_float2(a, a); }
+template <int OFF>
+__device__ __forceinline__ float4 lds128(const unsigned a) {  // 16 bytes from shared-window address a + OFF
+  float4 v;
+  asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4+%5];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(a), "n"(OFF) : "memory");
+  return v;
+}
 __device__ __forceinline__ float2 neg2(float2 a) { return make_float2(-a.x, -a.y); }
 
 struct SpeciesGrid {
@@ -168,8 +174,11 @@ __device__ __forceinline__ void fetch(const ChunkArgs& A, const WarpShared& sh, 
     if (BOTH) cu.flag = sh.flag[cu.cur];
   }
   m = cu.rec;
-  q = make_float4(0.f, 0.f, 0.f, 0.f);
-  if (pos < total) q = __ldg(A.pos4 + (__float_as_int(cu.rec.x) + pos));
+  // positions past the end of the stream sit on the closing dummy record, whose cell offset throws whatever is loaded
+  // 1e11 away: any valid address will do
+  (void)total;
+  q = __ldg(A.pos4 + min(__float_as_int(cu.rec.x) + pos, A.N - 1));
+
   if (BOTH) m.x = cu.flag;  // the slot offset has served; its place carries the species flag to to_frame
 }
 
@@ -180,7 +189,7 @@ __device__ __forceinline__ float4 to_frame(const float4 q, const float4 m, const
   s.x = fmaf(q.w + m.y, wxS, q.x);
   s.y = __fadd_rn(q.y, m.z);
   s.z = __fadd_rn(q.z, m.w);
-  s.w = BOTH ? m.x : 0.f;
+  s.w = BOTH ? m.x : q.w;  // (only BOTH streams read it)
   return s;
 }
 
@@ -203,16 +212,25 @@ __device__ __forceinline__ void run_stream(const ChunkArgs& A, const PairConsts&
   cu.flag = BOTH ? sh.flag[0] : 0.f;
   float4 q, m;
   fetch<BOTH>(A, sh, cu, lane, total, q, m);
-  float4* const wr = &sh.tile[0][lane];
-  const float4* const rd = &sh.tile[0][ph];
+  // shared-window addresses of this lane's store slot and first load slot; the double buffer is toggled by reflecting
+  // the address about the middle of the two buffers (one integer instruction each)
+  unsigned wr_a = (unsigned)__cvta_generic_to_shared(&sh.tile[0][lane]);
+  unsigned rd_a = (unsigned)__cvta_generic_to_shared(&sh.tile[0][ph]);
+  const unsigned wr_c = 2u * wr_a + 512u, rd_c = 2u * rd_a + 512u;
 #pragma unroll 1
   for (int i = 0; i < ntile; ++i) {
-    const int o = (i & 1) * 32;
-    wr[o] = to_frame<BOTH>(q, m, wxS);
+    const float4 s = to_frame<BOTH>(q, m, wxS);
+    asm volatile("st.shared.v4.f32 [%0], {%1, %2, %3, %4};" ::"r"(wr_a), "f"(s.x), "f"(s.y), "f"(s.z), "f"(s.w) : "memory");
     fetch<BOTH>(A, sh, cu, ((i + 1) << 5) + lane, total, q, m);
+
     __syncwarp();
-#pragma unroll
-    for (int j = 0; j < STEPS; ++j) evaluate<COUL, CUT, ENERGY, BOTH>(rd[o + NPH * j], t, acc, k, c);
+    static_assert(STEPS == 4, "written out for 4 steps per tile");
+    evaluate<COUL, CUT, ENERGY, BOTH>(lds128<0>(rd_a), t, acc, k, c);
+    evaluate<COUL, CUT, ENERGY, BOTH>(lds128<NPH * 16>(rd_a), t, acc, k, c);
+    evaluate<COUL, CUT, ENERGY, BOTH>(lds128<NPH * 32>(rd_a), t, acc, k, c);
+    evaluate<COUL, CUT, ENERGY, BOTH>(lds128<NPH * 48>(rd_a), t, acc, k, c);
+    wr_a = wr_c - wr_a;
+    rd_a = rd_c - rd_a;
   }
   __syncwarp();
   if (STATS && lane == 0) {
