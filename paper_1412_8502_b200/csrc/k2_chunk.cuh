@@ -7,17 +7,11 @@ namespace pasta {
 namespace {
 
 
-#define K2_T PASTA_CHUNK_T
-#ifndef K2_MINB
-#define K2_MINB 5
-#endif
-#ifndef K2_MINB_SPARSE
-#define K2_MINB_SPARSE 8
-#endif
-#ifndef K2_WARPS
-#define K2_WARPS 4
-#endif
-constexpr int T = K2_T;            // targets per chunk (4, 8 or 16)
+// Launch shape, settled by the sweeps of rounds 1 and 2 (profiles/r2_k2_experiments.md): 4 warps per
+// block; 5 resident blocks per SM (96 registers) where chunks stream hundreds of tiles, 8 (64 registers) where a species
+// is sparse and the latency of the listing sets the pace.
+constexpr int K2_MINB = 5, K2_MINB_SPARSE = 8, K2_WARPS = 4;
+constexpr int T = PASTA_CHUNK_T;   // targets per chunk
 constexpr int NPAIR = T / 2;       // packed target pairs per chunk
 constexpr int NPH = 32 / NPAIR;    // phases: lanes that share a target pair and split the sources of a tile
 constexpr int STEPS = 32 / NPH;    // sources a lane takes from each tile
