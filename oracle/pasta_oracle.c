@@ -13,7 +13,9 @@
  * Pins (tests/test_oracle_*.py, -m "not gpu"): closed-form two-particle table P1, finite
  * differences P2, np extremum P3, two-body oscillation period P4, Newton's third law P5,
  * translation/permutation invariance P6, all-pairs vs cell-list P7, dt^2 energy error P8,
- * thermostat P9, scaling P10, ideal-gas <PE> P11, neighbour count P12, cells P13, FoF P14.
+ * thermostat P9, scaling P10, ideal-gas <PE> P11, neighbour count P12, cells P13, FoF P14; the paper's own variants:
+ * r_nuc (range split), coul_nocut (Coulomb at the nearest image without a cut-off), linear box-only expansion,
+ * two-radius MST clusters, composition summary -- each by hand-built cases and invariants.
  * Parity unpinned: the paper's physics outputs (Table II, Figs. 3-9) -- unreachable run lengths.
  */
 #include <math.h>
