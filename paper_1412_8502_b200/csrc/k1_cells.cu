@@ -236,7 +236,9 @@ struct ChunkGeom {
   int nprim;     // primary entries
 };
 
-__device__ __forceinline__ void write_entry(int32_t* __restrict__ tab, int64_t e, int first, int n) {
+__device__ __forceinline__ void write_entry(int32_t* __restrict__ tab, int64_t e, int first, int n,
+                                            int32_t* __restrict__ chunk_first) {
+  for (int k = 0; k < n; ++k) chunk_first[first + k] = first;
 #pragma unroll
   for (int k = 0; k < CHUNK_T; k += 4) {
     int4 a;
@@ -250,7 +252,8 @@ __device__ __forceinline__ void write_entry(int32_t* __restrict__ tab, int64_t e
 
 __global__ void k1_chunk_rows_kernel(int32_t N, int32_t Np, const int32_t* __restrict__ cxyz,
                                      const int32_t* __restrict__ bin_start, const GridPair g, const ChunkGeom cg,
-                                     int32_t* __restrict__ chunk_tab, int32_t* __restrict__ n_overflow) {
+                                     int32_t* __restrict__ chunk_tab, int32_t* __restrict__ n_overflow,
+                                     int32_t* __restrict__ chunk_first) {
   const int j = blockIdx.x * blockDim.x + threadIdx.x;
   const int lo = j * CHUNK_T;
   if (lo >= N) return;
@@ -290,16 +293,16 @@ __global__ void k1_chunk_rows_kernel(int32_t N, int32_t Np, const int32_t* __res
       if (end) break;
     }
   }
-  write_entry(chunk_tab, j, m > 0 ? first_slot[0] : 0, m > 0 ? count[0] : 0);
+  write_entry(chunk_tab, j, m > 0 ? first_slot[0] : 0, m > 0 ? count[0] : 0, chunk_first);
   if (m > 1) {
     const int at = cg.nprim + atomicAdd(n_overflow, m - 1);
-    for (int k = 1; k < m; ++k) write_entry(chunk_tab, at + k - 1, first_slot[k], count[k]);
+    for (int k = 1; k < m; ++k) write_entry(chunk_tab, at + k - 1, first_slot[k], count[k], chunk_first);
   }
 }
 
 __global__ void k1_chunk_blocks_kernel(int sp, const int32_t* __restrict__ bin_start, const GridPair g,
                                        const ChunkGeom cg, int32_t* __restrict__ chunk_tab,
-                                       int32_t* __restrict__ n_overflow) {
+                                       int32_t* __restrict__ n_overflow, int32_t* __restrict__ chunk_first) {
   const int B = cg.block[sp], nc = g.ncell[sp], ncx = g.ncx[sp], xs = ncx / nc;
   const int nb = (nc + B - 1) / B;
   const int t = blockIdx.x * blockDim.x + threadIdx.x;
@@ -335,7 +338,9 @@ __global__ void k1_chunk_blocks_kernel(int sp, const int32_t* __restrict__ bin_s
       const int hi = __ldg(bs + x1);
       for (int p = __ldg(bs + x0); p < hi; ++p) out[k++] = p;
     }
+  const int n_real = k;
   for (; k < m * CHUNK_T; ++k) out[k] = -1;
+  for (k = 0; k < n_real; ++k) chunk_first[out[k]] = out[k - (k % CHUNK_T)];
 }
 
 // Cells per side of a species' grid: the O3 formula with the k that puts about CHUNK particles in a cell.
@@ -526,16 +531,18 @@ int k1_build(Sim* s, bool uniform_grid) {
     s->chunk_nprim = cg.nprim;
     s->max_chunks = cg.nprim + overflow;
     PASTA_TRY(buffer_reserve(s, &s->chunk_tab, sizeof(int32_t) * CHUNK_T * (size_t)(s->max_chunks + 8)));
+    PASTA_TRY(buffer_reserve(s, &s->chunk_first, sizeof(int32_t) * (size_t)N));
     if (any_rows) {
       k1_chunk_rows_kernel<<<grid_for(cg.nprim, 128), 128, 0, s->stream>>>(
-          (int32_t)N, (int32_t)s->Np, s->cxyz.as<int32_t>(), start, g, cg, s->chunk_tab.as<int32_t>(), n_overflow);
+          (int32_t)N, (int32_t)s->Np, s->cxyz.as<int32_t>(), start, g, cg, s->chunk_tab.as<int32_t>(), n_overflow,
+          s->chunk_first.as<int32_t>());
       s->launches += 1;
     }
     for (int sp = 0; sp < 2; ++sp)
       if (cg.block[sp] != 0 && (sp == 0 ? s->Np : N - s->Np) > 0) {
         const int64_t nb = (s->grid_sp[sp].ncell + cg.block[sp] - 1) / cg.block[sp];
-        k1_chunk_blocks_kernel<<<grid_for(nb * nb * nb, 128), 128, 0, s->stream>>>(sp, start, g, cg,
-                                                                                   s->chunk_tab.as<int32_t>(), n_overflow);
+        k1_chunk_blocks_kernel<<<grid_for(nb * nb * nb, 128), 128, 0, s->stream>>>(
+            sp, start, g, cg, s->chunk_tab.as<int32_t>(), n_overflow, s->chunk_first.as<int32_t>());
         s->launches += 1;
       }
   }

@@ -26,7 +26,10 @@ constexpr int CW = 4;  // warps (groups of 8 targets) per block
 
 struct CoulArgs {
   int32_t Np;
-  int32_t t_lo, t_hi;  // proton targets: sorted slots [t_lo, t_hi) (the whole range unless sharded)
+  int32_t t_lo, t_hi;  // proton slots the launch covers
+  int32_t w_lo, w_hi;  // target sharding: a target is evaluated iff its OWNER slot lies in [w_lo, w_hi)
+  const int32_t* owner;  // chunk path: first slot of the target's chunk (the rank that owns the chunk owns the target, so
+                         // that a particle is complete on one rank); NULL (list path): the target's own slot
   const float4* cpos;  // [2 Np] box fractions: [2 t] = hi parts (.w = 1), [2 t + 1] = lo parts
   const int32_t* perm;
   double* F;
@@ -109,6 +112,14 @@ __global__ void __launch_bounds__(CW * 32) k2c_pairs_kernel(const CoulArgs A) {
   const int t0 = A.t_lo + 8 * (blockIdx.x * CW + wib);
   if (t0 >= A.t_hi) return;
   const int ta = t0 + 2 * pr, tb = ta + 1;
+  bool mine[2];
+#pragma unroll
+  for (int k = 0; k < 2; ++k) {
+    const int ts = ta + k;
+    const int ow = ts < A.t_hi ? (A.owner ? __ldg(A.owner + ts) : ts) : -1;
+    mine[k] = ow >= A.w_lo && ow < A.w_hi;
+  }
+  if (!__any_sync(0xffffffffu, mine[0] || mine[1])) return;  // another rank's targets
   const int ca = 2 * min(ta, A.Np - 1), cb = 2 * min(tb, A.Np - 1);
   const float4 pa = __ldg(A.cpos + ca), pb = __ldg(A.cpos + cb), qa = __ldg(A.cpos + ca + 1), qb = __ldg(A.cpos + cb + 1);
   CTargets t;
@@ -143,7 +154,7 @@ __global__ void __launch_bounds__(CW * 32) k2c_pairs_kernel(const CoulArgs A) {
 #pragma unroll
     for (int k = 0; k < 2; ++k) {
       const int ts = ta + k;
-      if (ts < A.t_hi) {
+      if (mine[k]) {
         const int64_t i = __ldg(A.perm + ts);
         A.F[3 * i + 0] -= A.aL * v[4 * k + 0];  // du was u_j - u_i
         A.F[3 * i + 1] -= A.aL * v[4 * k + 1];
@@ -166,8 +177,13 @@ int k2_coulomb_all_pairs(Sim* s, bool with_energy) {
   PASTA_TRY(buffer_reserve(s, &s->cpos, 2 * sizeof(float4) * (size_t)s->Np));
   CoulArgs A;
   A.Np = (int32_t)s->Np;
-  A.t_lo = s->shard.slot_lo < 0 ? 0 : s->shard.slot_lo;
-  A.t_hi = s->shard.slot_hi > A.Np ? A.Np : s->shard.slot_hi;
+  A.w_lo = s->shard.slot_lo;
+  A.w_hi = s->shard.slot_hi;
+  A.owner = s->sort_kind == 0 ? s->chunk_first.as<int32_t>() : nullptr;
+  // list path: a target is owned through its own slot, so the launch covers the window only; chunk path: every
+  // proton group looks its owner up and the others' return at once
+  A.t_lo = A.owner ? 0 : (s->shard.slot_lo < 0 ? 0 : s->shard.slot_lo);
+  A.t_hi = A.owner ? A.Np : (s->shard.slot_hi > A.Np ? A.Np : s->shard.slot_hi);
   A.cpos = s->cpos.as<float4>();
   A.perm = s->perm.as<int32_t>();
   A.F = s->F.as<double>();

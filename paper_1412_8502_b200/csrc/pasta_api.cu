@@ -58,7 +58,7 @@ void buffer_release(Sim* s, Buffer* b) {
 static void release_all(Sim* s) {
   Buffer* bs[] = {&s->x, &s->v, &s->F, &s->e, &s->is_p, &s->cell_id, &s->bin_count, &s->bin_start, &s->scan_tmp,
                   &s->perm, &s->perm_raw, &s->pos4, &s->cxyz, &s->cpos, &s->partials, &s->scalars, &s->counters, &s->cl_parent, &s->cl_A,
-                  &s->cl_Z, &s->cl_cell_id, &s->cl_count, &s->cl_start, &s->cl_perm, &s->chunk_tab, &s->xref, &s->slot_of, &s->list_off,
+                  &s->cl_Z, &s->cl_cell_id, &s->cl_count, &s->cl_start, &s->cl_perm, &s->chunk_tab, &s->chunk_first, &s->xref, &s->slot_of, &s->list_off,
                   &s->list_pool};
   for (Buffer* b : bs) buffer_release(s, b);
 }

@@ -240,6 +240,7 @@ struct Sim {
   // [max_chunks, 2 max_chunks) the list of chunks that need several rounds; the counters live in
   // counters[24] (int32 view [48]: number of chunks, [49]: length of that list)
   Buffer chunk_tab;
+  Buffer chunk_first;       // int32[N]: first target slot of the chunk a sorted slot belongs to (who owns it under sharding)
   int64_t max_chunks = 0;   // launch bound of the pair kernel: chunk_nprim primary entries + overflow capacity
   int64_t chunk_nprim = 0;
   bool chunks_sparse = false;  // some species' chunks come from the SPARSE (cell block) builder

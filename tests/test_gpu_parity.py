@@ -756,7 +756,8 @@ def test_random_small_systems(orc, seed):
     assert abs(pairs - d["ordered_pairs"]) <= 4
 
 
-def test_captured_step_equals_kernel_by_kernel(monkeypatch):
+@pytest.mark.parametrize("paper_mode", [False, True])
+def test_captured_step_equals_kernel_by_kernel(monkeypatch, paper_mode):
     """a fixed-box step is captured as a CUDA graph after two warm steps and replayed with one launch.
     The replay must (i) really happen, (ii) leave positions, velocities, forces and the kinetic energy BIT-identical to
     the kernel-by-kernel path (PASTA_GRAPHS=0), across rescale steps (interval 10: both graphs are used), across a
@@ -767,6 +768,8 @@ def test_captured_step_equals_kernel_by_kernel(monkeypatch):
     for graphs in ("1", "0"):
         monkeypatch.setenv("PASTA_GRAPHS", graphs)
         p = pasta.default_params(r_c=c["r_c"], thermostat_interval=10)
+        if paper_mode:  # the all-pairs Coulomb kernels are captured with the rest
+            p.r_nuc, p.coulomb_all_pairs = 11.5, 1
         with pasta.Sim(8192, 0.3, 0.05, 1.0, params=p, seed=11) as sim:
             sim.step(25, 2.0)
             r0 = sim.graph_replays()

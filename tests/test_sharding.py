@@ -76,13 +76,15 @@ def test_partition_world_size_2_gloo(tmp_path):
 
 
 @pytest.mark.gpu
-@pytest.mark.parametrize("cfg_like,world", [((20000, 0.3, 0.05, 17.0), 3), ((30000, 0.05, 0.002, 20.0), 4)])
-def test_ranks_played_in_turn_add_up_bit_exactly(cfg_like, world):
-    """Dense chunk path and (second case: cold, dilute, wide box) the neighbour-list path."""
+@pytest.mark.parametrize("cfg_like,world,paper_mode", [((20000, 0.3, 0.05, 17.0), 3, False), ((30000, 0.05, 0.002, 20.0), 4, False),
+                                                       ((20000, 0.4, 0.01, 20.0), 3, True)])
+def test_ranks_played_in_turn_add_up_bit_exactly(cfg_like, world, paper_mode):
+    """Dense chunk path, (second case: cold, dilute, wide box) the neighbour-list path, and (third) the paper's range
+    split with the all-pairs Coulomb kernel, whose proton targets are sharded by the same window."""
     import torch
 
     N, Y_P, density, r_c = cfg_like
-    p = pasta.default_params(r_c=r_c)
+    p = pasta.default_params(r_c=r_c, r_nuc=11.5, coulomb_all_pairs=1) if paper_mode else pasta.default_params(r_c=r_c)
     with pasta.Sim(N, Y_P, density, 0.5, params=p, seed=5) as sim:
         F1, pe1 = sim.forces()
         e1 = sim.particle_energies().clone()
@@ -95,13 +97,15 @@ def test_ranks_played_in_turn_add_up_bit_exactly(cfg_like, world):
             eparts.append(sim.particle_energies().clone())
         assert calls == [3 * N, N] * world
         owners = sum((q != 0).any(dim=1).to(torch.int32) for q in parts)
-        assert int(owners.max()) == 1 and int((owners == 0).sum()) <= 2        # every particle on exactly one rank
+        # every particle on exactly one rank (in the paper's mode too: the all-pairs Coulomb kernel takes a proton's owner
+        # from its chunk, so that nuclear and Coulomb parts are added on one rank in the one-GPU order)
+        assert int(owners.max()) == 1 and int((owners == 0).sum()) <= 2
         assert torch.equal(sum(parts), F1) and torch.equal(sum(eparts), e1)
         Np = int(sim.get_state()[2].sum())
         b = pasta.shard_bounds(N, Np, *sim.shard_costs(), world)
         sizes = [int((q != 0).any(dim=1).sum()) for q in parts]
         # ownership goes by a chunk's FIRST target; a chunk of the cell-block builder gathers slots of several rows
-        assert sum(sizes) >= N - 2 and all(abs(sizes[r] - (b[r + 1] - b[r])) <= 0.05 * N for r in range(world))
+        assert N - 2 <= sum(sizes) <= N and all(abs(sizes[r] - (b[r + 1] - b[r])) <= 0.05 * N for r in range(world))
         sim.set_shard(0, 1)
         F, pe = sim.forces()
         assert torch.equal(F, F1) and pe == pe1
