@@ -826,3 +826,23 @@ def test_coulomb_without_cutoff_mode(orc, N, Y_P, density, path):
         assert (sim.list_stats()["list_builds"] < sim.list_stats()["force_evals"]) == (path == "list")
     with pytest.raises(pasta.PastaError):
         pasta.Sim(N, Y_P, density, 1.0, params=pasta.default_params(coulomb_all_pairs=1), seed=1)
+
+
+@pytest.mark.parametrize("N,Y_P,density,extra", [(8192, 0.3, 0.05, {}), (20000, 0.2, 0.00125, {}),
+                                                 (8192, 0.4, 0.004, {"r_nuc": 11.5, "coulomb_all_pairs": 1})])
+def test_steps_without_per_step_energies(N, Y_P, density, extra):
+    """pasta_params.energy_every_step = 0: the pair kernels skip the energy terms during pasta_step.  The forces, and
+    with them the trajectory, must be BIT-identical to a run that evaluates the energies every step (chunk path, list
+    path, the paper's mode), and pasta_energy / pasta_particle_energies must still return the energies of the final
+    configuration (they re-evaluate on demand)."""
+    out = []
+    for every in (1, 0):
+        p = pasta.default_params(r_c=20.0 if N > 10000 or extra else 17.0, thermostat_interval=4, energy_every_step=every, **extra)
+        with pasta.Sim(N, Y_P, density, 0.5, params=p, seed=17) as sim:
+            sim.step(11, 2.0)
+            x, v, _, L, _ = sim.get_state()
+            ke, pe = sim.energy()
+            out.append((x.clone(), v.clone(), ke, pe, sim.particle_energies().clone()))
+    a, b = out
+    assert _torch().equal(a[0], b[0]) and _torch().equal(a[1], b[1])
+    assert a[2] == b[2] and a[3] == b[3] and _torch().equal(a[4], b[4])
