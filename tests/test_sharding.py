@@ -119,17 +119,26 @@ import paper_1412_8502_b200 as pasta
 dist.init_process_group("gloo")
 rank, world = dist.get_rank(), dist.get_world_size()
 torch.cuda.set_device(0)                      # both ranks share the one GPU; only the HOST waits in the collective
-p = pasta.default_params(r_c=17.0, thermostat_interval=5)
-sim = pasta.Sim(6000, 0.3, 0.05, 1.0, params=p, seed=3)
-if world > 1:
-    sim.set_shard(rank, world)
-sim.step(12, 2.0)
-x, v, _, L, step = sim.get_state()
-F, pe = sim.forces()
+cases = {
+    "dense": (6000, 0.3, 0.05, dict(r_c=17.0, thermostat_interval=5), 12),
+    "dilute_lists_scaling_box": (8000, 0.2, 0.001, dict(r_c=20.0, thermostat_interval=5, scale_per_step=1.0004), 40),
+    "paper_mode": (5000, 0.4, 0.003, dict(r_c=20.0, r_nuc=11.5, coulomb_all_pairs=1, thermostat_interval=4), 10),
+}
+out = {}
+for name, (N, Y_P, density, prm, steps) in cases.items():
+    sim = pasta.Sim(N, Y_P, density, 0.5, params=pasta.default_params(**prm), seed=3)
+    if world > 1:
+        sim.set_shard(rank, world)
+    sim.step(steps, 2.0)
+    x, v, _, L, step = sim.get_state()
+    F, pe = sim.forces()
+    ke, pe2 = sim.energy()
+    out[name] = {"x": x.cpu(), "v": v.cpu(), "F": F.cpu(), "pe": pe, "ke": ke, "L": L, "stats": sim.list_stats()}
+    dist.barrier()
+    sim.close()
 if rank == 0:
-    torch.save({"x": x.cpu(), "v": v.cpu(), "F": F.cpu(), "pe": pe}, sys.argv[1])
+    torch.save(out, sys.argv[1])
 dist.barrier()
-sim.close()
 dist.destroy_process_group()
 """
 
@@ -148,6 +157,9 @@ def test_two_sharded_processes_reproduce_the_unsharded_trajectory(tmp_path):
         out = subprocess.run(cmd, capture_output=True, text=True, timeout=600, env=dict(os.environ, OMP_NUM_THREADS="1"))
         assert out.returncode == 0, out.stderr[-3000:]
         res[world] = torch.load(out_file)
-    for k in ("x", "v", "F"):
-        assert torch.equal(res[1][k], res[2][k]), k
-    assert res[1]["pe"] == res[2]["pe"]
+    for case in res[1]:
+        one, two = res[1][case], res[2][case]
+        for k in ("x", "v", "F"):
+            assert torch.equal(one[k], two[k]), (case, k)
+        assert one["pe"] == two["pe"] and one["ke"] == two["ke"] and one["L"] == two["L"] and one["stats"] == two["stats"], case
+    assert res[1]["dilute_lists_scaling_box"]["stats"]["list_builds"] < 20   # that case really ran on reused lists
