@@ -78,7 +78,7 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) k2_chunk_kernel(const ChunkA
 
 }  // namespace
 
-int k2_chunk_forces(Sim* s, bool with_energy, bool stats) {
+int k2_chunk_forces(Sim* s, bool with_energy, bool stats, double kick) {
   const PairConsts c = make_pair_consts(s->prm);
   const double sigma = sqrt(1.4426950408889634074 / (2.0 * s->prm.Lambda));
   if (s->N >= (1ll << 26)) {
@@ -116,6 +116,8 @@ int k2_chunk_forces(Sim* s, bool with_energy, bool stats) {
   A.perm = s->perm.as<int32_t>();
   A.F = s->F.as<double>();
   A.e = s->e.as<double>();
+  A.v = s->v.as<double>();
+  A.kick = kick;
   A.stats = s->counters.as<unsigned long long>() + 10;
   // exp2(-r'^2) is exactly 0 (FTZ) for r'^2 > 126: then np/nn pairs beyond r_c need no explicit cut
   const bool cut = (double)c.rn2s < 127.0;  // the nuclear cut-off lies inside the FP32 underflow distance

@@ -64,6 +64,8 @@ struct ChunkArgs {
   const int32_t* perm;
   double* F;
   double* e;
+  double* v;       // kick != 0: the second half kick v += kick F rides along with the force write (O2 step 4)
+  double kick;
   unsigned long long* stats;  // [0] sources streamed, [1] tiles, [2] pair evaluations (STATS only)
 };
 
@@ -489,7 +491,9 @@ __device__ __forceinline__ void write_chunk_results(const ChunkArgs& A, const Pa
     if (ph < L8 && tgt_slot >= 0) {
       const int i = __ldg(A.perm + tgt_slot);
       if (comp < 3) {
-        A.F[3 * (int64_t)i + comp] = -v[j];  // d was x_j - x_i
+        const double Fc = -v[j];  // d was x_j - x_i
+        A.F[3 * (int64_t)i + comp] = Fc;
+        if (A.kick != 0.0) A.v[3 * (int64_t)i + comp] = A.v[3 * (int64_t)i + comp] + A.kick * Fc;  // as k3_kick_ke_kernel
       } else if (ENERGY) {
         // every target met itself once in its own species' pass at r = 0: remove V(0) = a + b + c
         A.e[i] = 0.5 * (v[j] - (double)c.v_self);

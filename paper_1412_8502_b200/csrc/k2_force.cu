@@ -211,10 +211,16 @@ static V0Args make_v0_args(Sim* s) {
   return A;
 }
 
-int k2_forces(Sim* s, bool with_energy) {
+int k2_forces(Sim* s, bool with_energy, double kick) {
   // force_variant: 0 = library default (chunk kernel), 1 = thread-per-target reference, 2 = chunk kernel
-  if (s->tune.force_variant == 1) return k2_reference_forces(s, with_energy);
-  return k2_chunk_forces(s, with_energy, false);
+  if (s->tune.force_variant == 1) {
+    if (kick != 0.0) {
+      set_error("the thread-per-target kernel has no fused kick");
+      return PASTA_ESTATE;
+    }
+    return k2_reference_forces(s, with_energy);
+  }
+  return k2_chunk_forces(s, with_energy, false, kick);
 }
 
 int k2_reference_forces(Sim* s, bool with_energy) {

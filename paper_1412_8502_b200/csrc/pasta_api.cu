@@ -128,7 +128,7 @@ static int shard_window(Sim* s) {
   return PASTA_OK;
 }
 
-static int evaluate_forces_tail(Sim* s, bool with_energy) {
+static int evaluate_forces_tail(Sim* s, bool with_energy, double kick = 0.0) {
   s->n_force_evals += 1;
   const bool sharded = s->shard.world > 1;
   PASTA_TRY(shard_window(s));
@@ -139,7 +139,7 @@ static int evaluate_forces_tail(Sim* s, bool with_energy) {
       if (with_energy) PASTA_CUDA_OK(cudaMemsetAsync(s->e.ptr, 0, 8 * (size_t)s->N, s->stream));
     }
     if (s->list.valid) PASTA_TRY(k2_list_forces(s, with_energy));
-    else PASTA_TRY(k2_forces(s, with_energy));
+    else PASTA_TRY(k2_forces(s, with_energy, kick));
     if (s->prm.coulomb_all_pairs) PASTA_TRY(k2_coulomb_all_pairs(s, with_energy));
     if (sharded) {
       if (s->shard.allreduce(s->F.ptr, 3 * s->N, s->shard.user) != 0 ||
@@ -155,7 +155,11 @@ static int evaluate_forces_tail(Sim* s, bool with_energy) {
   return PASTA_OK;
 }
 
-static int evaluate_forces(Sim* s, bool with_energy) {
+// kick != 0 (a caller that has checked kick_can_ride): the chunk kernel adds v += kick F as it writes F.
+static bool kick_can_ride(const Sim* s) {
+  return s->tune.force_variant == 0 && s->shard.world <= 1 && !s->prm.coulomb_all_pairs && !s->list.valid && !list_mode_wanted(s);
+}
+static int evaluate_forces(Sim* s, bool with_energy, double kick = 0.0) {
   {
     Timer t(s, 0);
     if (s->list.valid) {
@@ -188,11 +192,9 @@ static int evaluate_forces(Sim* s, bool with_energy) {
       }
     }
   }
-  return evaluate_forces_tail(s, with_energy);
+  return evaluate_forces_tail(s, with_energy, kick);
 }
 
-// One MD step with s->L already set to the box the forces are evaluated in (O2: first half kick + drift, forces,
-// second half kick, rescale on every thermostat_interval-th step).
 // A step on reused neighbour lists without a round trip to the host in its critical path: the
 // kick-drift kernel refreshes the frozen order, measures the largest displacement since the build and DECIDES on the
 // device whether the lists survive (2 D <= halo); the force kernel -- with the second half kick riding along -- is
@@ -259,9 +261,12 @@ static int step_body(Sim* s, double dt, double sc, double L_wrap, bool energy, b
     s->lin_n += 1;
   }
   s->clusters_valid = false;
-  PASTA_TRY(evaluate_forces(s, energy));
+  // a plain step on the chunk path: the second half kick rides along with the force write of the pair kernel; a step
+  // that ends with the rescale needs the kinetic energy and keeps the kick kernel
+  const bool ride = !rescale && kick_can_ride(s);
+  PASTA_TRY(evaluate_forces(s, energy, ride ? dt / (2.0 * s->prm.mass) : 0.0));
   s->step_count += 1;
-  {
+  if (!ride) {
     Timer t(s, 2);
     PASTA_TRY(k3_kick_ke(s, dt, rescale));
   }

@@ -301,10 +301,10 @@ int k1_build(Sim* s, bool uniform_grid = false);       // (species,cell) countin
 int k1_export_cells(Sim* s, int32_t* cell_id_dev, int32_t* cell_start_dev);
 int scan_exclusive(Sim* s, const int32_t* in, int32_t* out, int64_t n);  // out[0..n] (n+1 entries)
 // K2  k2_force.cu
-int k2_forces(Sim* s, bool with_energy);               // F, e in original order
+int k2_forces(Sim* s, bool with_energy, double kick = 0.0);  // F, e in original order; kick != 0: v += kick F rides along
 int k2_pair_count(Sim* s, int64_t* ordered_pairs_host, int64_t* nonzero_pairs_host);
 int k2_reference_forces(Sim* s, bool with_energy);     // variant 1: thread per target (k2_force.cu)
-int k2_chunk_forces(Sim* s, bool with_energy, bool stats);  // variant 2: chunk kernel (k2_chunk.cu)
+int k2_chunk_forces(Sim* s, bool with_energy, bool stats, double kick = 0.0);  // variant 2: chunk kernel (k2_chunk.cu)
 int k2_list_build(Sim* s, double halo);                // neighbour lists of the sorted order k1_build just made (k2_list.cu)
 int k2_list_forces(Sim* s, bool with_energy, bool gated = false, double kick = 0.0);  // the pair kernel on those lists; gated:
                                                        // only if the refresh just enqueued lets the lists live; kick: v += kick F
