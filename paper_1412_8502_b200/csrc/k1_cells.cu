@@ -145,8 +145,10 @@ int scan_exclusive(Sim* s, const int32_t* in, int32_t* out, int64_t n) {
 }
 
 __global__ void k1_scatter_kernel(int64_t N, const int32_t* __restrict__ pbin, const int32_t* __restrict__ bin_start,
-                                  int32_t* __restrict__ bin_count, int32_t* __restrict__ perm) {
+                                  int32_t* __restrict__ bin_count, int32_t* __restrict__ perm,
+                                  int32_t* __restrict__ zero_me) {
   int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i == 0 && zero_me) *zero_me = 0;  // the overflow counter of the chunk table (the kernels behind this one add to it)
   if (i >= N) return;
   const int bin = pbin[i];
   const int old = atomicSub(&bin_count[bin], 1);  // leaves the histogram zeroed for the next build
@@ -176,43 +178,62 @@ __global__ void k1_order_kernel(int64_t nbins, const int32_t* __restrict__ bin_s
 // arrival order was, and writes it to `perm_out`.  (Thin-cell bins hold a particle or two; the uniform one-grid
 // variant, whose bins hold hundreds, orders them with k1_order_kernel instead.)
 // list_format (k2_list.cu): pos4.w carries the bits of the packed cell coordinates instead of the thin-cell index as a float.
+struct GatherArgs {
+  int64_t N;
+  const double* x;
+  const int32_t* pbin;
+  const int32_t* perm_in;
+  int32_t* perm_out;
+  const int32_t* bin_start;
+  GridPair g;
+  double sigma;
+  float4* pos4;
+  int32_t* cxyz;
+  bool list_format;
+  int32_t* slot_of;
+};
+__device__ __forceinline__ int packed_cell_of_bin(const GridPair& g, const int bin) {
+  const int sp = bin >= g.base[1] ? 1 : 0;
+  const int id = bin - g.base[sp], nc = g.ncell[sp], ncx = g.ncx[sp];
+  return (id % ncx) | (((id / ncx) % nc) << 12) | ((id / (ncx * nc)) << 22);
+}
+// Sorted slot t (t < N); returns its packed cell coordinates.
 template <bool FUSED_ORDER>
-__global__ void k1_gather_kernel(int64_t N, const double* __restrict__ x, const int32_t* __restrict__ pbin,
-                                 const int32_t* __restrict__ perm_in, int32_t* __restrict__ perm_out,
-                                 const int32_t* __restrict__ bin_start, const GridPair g, double sigma,
-                                 float4* __restrict__ pos4, int32_t* __restrict__ cxyz,
-                                 int32_t* __restrict__ zero_me, bool list_format, int32_t* __restrict__ slot_of) {
-  int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-  if (t == 0 && zero_me) *zero_me = 0;  // the overflow counter of the chunk table
-  if (t >= N) return;
-  int i = perm_in[t];
-  const int bin = pbin[i];
+__device__ __forceinline__ int gather_slot(const GatherArgs& G, const int64_t t) {
+  int i = G.perm_in[t];
+  const int bin = G.pbin[i];
   if (FUSED_ORDER) {
-    const int lo = bin_start[bin], hi = bin_start[bin + 1];
+    const int lo = G.bin_start[bin], hi = G.bin_start[bin + 1];
     if (hi - lo > 1) {
       const int want = (int)t - lo;
       for (int a = lo; a < hi; ++a) {
-        const int ia = perm_in[a];
+        const int ia = G.perm_in[a];
         int rank = 0;
-        for (int b = lo; b < hi; ++b) rank += perm_in[b] < ia ? 1 : 0;
+        for (int b = lo; b < hi; ++b) rank += G.perm_in[b] < ia ? 1 : 0;
         if (rank == want) i = ia;
       }
     }
-    perm_out[t] = i;
+    G.perm_out[t] = i;
   }
-  if (slot_of) slot_of[i] = (int32_t)t;
+  if (G.slot_of) G.slot_of[i] = (int32_t)t;
+  const GridPair& g = G.g;
   const int sp = bin >= g.base[1] ? 1 : 0;
-  const int id = bin - g.base[sp], nc = g.ncell[sp], ncx = g.ncx[sp];
+  const int packed = packed_cell_of_bin(g, bin);
+  const int cx = PASTA_CX(packed), cy = PASTA_CY(packed), cz = PASTA_CZ(packed);
   const double w = g.w[sp];
-  const int cx = id % ncx, cy = (id / ncx) % nc, cz = id / (ncx * nc);
   float4 p;
-  p.x = (float)(sigma * (x[3 * i + 0] - ((double)cx + 0.5) * g.wx[sp]));
-  p.y = (float)(sigma * (x[3 * i + 1] - ((double)cy + 0.5) * w));
-  p.z = (float)(sigma * (x[3 * i + 2] - ((double)cz + 0.5) * w));
-  const int packed = cx | (cy << 12) | (cz << 22);
-  p.w = list_format ? __int_as_float(packed) : (float)cx;
-  pos4[t] = p;
-  cxyz[t] = packed;
+  p.x = (float)(G.sigma * (G.x[3 * i + 0] - ((double)cx + 0.5) * g.wx[sp]));
+  p.y = (float)(G.sigma * (G.x[3 * i + 1] - ((double)cy + 0.5) * w));
+  p.z = (float)(G.sigma * (G.x[3 * i + 2] - ((double)cz + 0.5) * w));
+  p.w = G.list_format ? __int_as_float(packed) : (float)cx;
+  G.pos4[t] = p;
+  G.cxyz[t] = packed;
+  return packed;
+}
+template <bool FUSED_ORDER>
+__global__ void k1_gather_kernel(const GatherArgs G) {
+  const int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (t < G.N) gather_slot<FUSED_ORDER>(G, t);
 }
 
 // Chunk table of the pair kernel.  A chunk = the targets of one warp = up to CHUNK_T sorted slots of one species
@@ -250,11 +271,12 @@ __device__ __forceinline__ void write_entry(int32_t* __restrict__ tab, int64_t e
   }
 }
 
-__global__ void k1_chunk_rows_kernel(int32_t N, int32_t Np, const int32_t* __restrict__ cxyz,
-                                     const int32_t* __restrict__ bin_start, const GridPair g, const ChunkGeom cg,
-                                     int32_t* __restrict__ chunk_tab, int32_t* __restrict__ n_overflow,
-                                     int32_t* __restrict__ chunk_first) {
-  const int j = blockIdx.x * blockDim.x + threadIdx.x;
+// Entry j of the DENSE builder; cell_of(p) = packed cell coordinates of sorted slot p (p < N).
+template <class CellOf>
+__device__ __forceinline__ void chunk_rows_entry(const int j, const int32_t N, const int32_t Np, CellOf cell_of,
+                                                 const int32_t* __restrict__ bin_start, const GridPair& g,
+                                                 const ChunkGeom& cg, int32_t* __restrict__ chunk_tab,
+                                                 int32_t* __restrict__ n_overflow, int32_t* __restrict__ chunk_first) {
   const int lo = j * CHUNK_T;
   if (lo >= N) return;
   // row key of a slot: species and (cy, cz); -1 beyond the end
@@ -262,7 +284,7 @@ __global__ void k1_chunk_rows_kernel(int32_t N, int32_t Np, const int32_t* __res
 #pragma unroll
   for (int k = 0; k < 2 * CHUNK_T; ++k) {
     const int p = lo + k;
-    c[k] = p < N ? __ldg(cxyz + p) : 0;
+    c[k] = p < N ? cell_of(p) : 0;
     key[k] = p < N ? ((c[k] >> 12) | (p < Np ? 0 : (1 << 24))) : -1;
   }
   // first slot of the row that slot `lo` belongs to
@@ -297,6 +319,29 @@ __global__ void k1_chunk_rows_kernel(int32_t N, int32_t Np, const int32_t* __res
   if (m > 1) {
     const int at = cg.nprim + atomicAdd(n_overflow, m - 1);
     for (int k = 1; k < m; ++k) write_entry(chunk_tab, at + k - 1, first_slot[k], count[k], chunk_first);
+  }
+}
+
+// The gather and the DENSE chunk builder in one launch: a block gathers 256 sorted slots, keeps their packed cell
+// coordinates in shared memory together with those of the 16 slots behind them (their bins are known from the scatter,
+// whatever the order inside a bin will be), and its first 32 threads then write the 32 table entries of these slots.
+constexpr int GATHER_T = 256;
+__global__ void __launch_bounds__(GATHER_T) k1_gather_chunks_kernel(const GatherArgs G, const int32_t Np, const ChunkGeom cg,
+                                                                    int32_t* __restrict__ chunk_tab,
+                                                                    int32_t* __restrict__ n_overflow,
+                                                                    int32_t* __restrict__ chunk_first) {
+  __shared__ int cell[GATHER_T + 2 * CHUNK_T];
+  const int64_t base = (int64_t)blockIdx.x * GATHER_T, t = base + threadIdx.x;
+  if (t < G.N) cell[threadIdx.x] = gather_slot<true>(G, t);
+  if (threadIdx.x < 2 * CHUNK_T) {
+    const int64_t u = base + GATHER_T + threadIdx.x;
+    if (u < G.N) cell[GATHER_T + threadIdx.x] = packed_cell_of_bin(G.g, G.pbin[G.perm_in[u]]);
+  }
+  __syncthreads();
+  if (threadIdx.x < GATHER_T / CHUNK_T) {
+    const int j = blockIdx.x * (GATHER_T / CHUNK_T) + threadIdx.x;
+    chunk_rows_entry(j, (int32_t)G.N, Np, [&](int p) { return cell[p - (int)base]; }, G.bin_start, G.g, cg, chunk_tab,
+                     n_overflow, chunk_first);
   }
 }
 
@@ -477,30 +522,35 @@ int k1_build(Sim* s, bool uniform_grid) {
   PASTA_TRY(scan_exclusive(s, cnt, start, nbins));
   const double sigma = sqrt(1.4426950408889634074 / (2.0 * s->prm.Lambda));
   int32_t* n_overflow = s->counters.as<int32_t>() + 2 * 24;
+  GatherArgs G;
+  G.N = N;
+  G.x = s->x.as<double>();
+  G.pbin = s->cell_id.as<int32_t>();
+  G.bin_start = start;
+  G.g = g;
+  G.sigma = sigma;
+  G.pos4 = s->pos4.as<float4>();
+  G.cxyz = s->cxyz.as<int32_t>();
+  G.list_format = lists;
+  G.slot_of = nullptr;
   if (uniform) {
-    k1_scatter_kernel<<<grid_for(N, B), B, 0, s->stream>>>(N, s->cell_id.as<int32_t>(), start, cnt, s->perm.as<int32_t>());
+    G.perm_in = s->perm.as<int32_t>();
+    G.perm_out = nullptr;
+    k1_scatter_kernel<<<grid_for(N, B), B, 0, s->stream>>>(N, G.pbin, start, cnt, s->perm.as<int32_t>(), nullptr);
     k1_order_kernel<<<grid_for(nbins, B), B, 0, s->stream>>>(nbins, start, s->perm.as<int32_t>());
-    k1_gather_kernel<false><<<grid_for(N, B), B, 0, s->stream>>>(N, s->x.as<double>(), s->cell_id.as<int32_t>(),
-                                                                 s->perm.as<int32_t>(), nullptr, start, g, sigma,
-                                                                 s->pos4.as<float4>(), s->cxyz.as<int32_t>(), nullptr, false, nullptr);
+    k1_gather_kernel<false><<<grid_for(N, B), B, 0, s->stream>>>(G);
     s->launches += 3;
   } else {
-    if (lists) PASTA_TRY(buffer_reserve(s, &s->slot_of, sizeof(int32_t) * (size_t)N));
-    k1_scatter_kernel<<<grid_for(N, B), B, 0, s->stream>>>(N, s->cell_id.as<int32_t>(), start, cnt,
-                                                           s->perm_raw.as<int32_t>());
-    k1_gather_kernel<true><<<grid_for(N, B), B, 0, s->stream>>>(N, s->x.as<double>(), s->cell_id.as<int32_t>(),
-                                                                s->perm_raw.as<int32_t>(), s->perm.as<int32_t>(), start,
-                                                                g, sigma, s->pos4.as<float4>(), s->cxyz.as<int32_t>(),
-                                                                n_overflow, lists, lists ? s->slot_of.as<int32_t>() : nullptr);
-    s->launches += 2;
-  }
-  if (!uniform && !lists) {
-    // builder per species (DENSE row runs: at least 3 particles per cell on average), the extent limit of a row
-    // run (three cell widths, at most 16 fm) and the capacity of the table: a bound on the number of chunks
+    G.perm_in = s->perm_raw.as<int32_t>();
+    G.perm_out = s->perm.as<int32_t>();
+    // the chunk table of the pair kernel (not in list mode): builder per species (DENSE row runs: at least 3
+    // particles per cell on average), the extent limit of a row run (three cell widths, at most 16 fm) and the
+    // capacity of the table: a bound on the number of chunks
     //   row runs: primary entries ceil(N / 8); overflow <= one per row (row or species change inside 8 slots)
     //             + ncx / xmax + 1 per row (runs cut at the extent limit cover disjoint stretches >= xmax)
     //   blocks:   n / 8 + one per block
     ChunkGeom cg;
+    cg.nprim = 0;
     int64_t overflow = 64;
     bool any_rows = false;
     for (int sp = 0; sp < 2; ++sp) {
@@ -511,11 +561,11 @@ int k1_build(Sim* s, bool uniform_grid) {
       cg.xmax[sp] = xm < 1 ? 1 : xm;
       cg.block[sp] = 0;
       if (occ < 3.0 && gr.ncell >= 4) {
-        int B = (int)ceil(cbrt(8.0 / fmax(occ, 1e-9)));
+        int Bb = (int)ceil(cbrt(8.0 / fmax(occ, 1e-9)));
         const int Bmax = (int)floor(20.0 / gr.w);
-        B = B > 3 ? 3 : B;
-        B = B > Bmax ? Bmax : B;
-        cg.block[sp] = B < 1 ? 1 : B;
+        Bb = Bb > 3 ? 3 : Bb;
+        Bb = Bb > Bmax ? Bmax : Bb;
+        cg.block[sp] = Bb < 1 ? 1 : Bb;
       }
       const int64_t nrow = (int64_t)gr.ncell * gr.ncell;
       if (cg.block[sp] == 0) {
@@ -526,25 +576,36 @@ int k1_build(Sim* s, bool uniform_grid) {
         overflow += n_sp / CHUNK_T + nb * nb * nb;
       }
     }
-    cg.nprim = any_rows ? (int)((N + CHUNK_T - 1) / CHUNK_T) : 0;
-    s->chunks_sparse = (cg.block[0] != 0 && s->Np > 0) || (cg.block[1] != 0 && N - s->Np > 0);
-    s->chunk_nprim = cg.nprim;
-    s->max_chunks = cg.nprim + overflow;
-    PASTA_TRY(buffer_reserve(s, &s->chunk_tab, sizeof(int32_t) * CHUNK_T * (size_t)(s->max_chunks + 8)));
-    PASTA_TRY(buffer_reserve(s, &s->chunk_first, sizeof(int32_t) * (size_t)N));
-    if (any_rows) {
-      k1_chunk_rows_kernel<<<grid_for(cg.nprim, 128), 128, 0, s->stream>>>(
-          (int32_t)N, (int32_t)s->Np, s->cxyz.as<int32_t>(), start, g, cg, s->chunk_tab.as<int32_t>(), n_overflow,
-          s->chunk_first.as<int32_t>());
-      s->launches += 1;
+    if (lists) {
+      PASTA_TRY(buffer_reserve(s, &s->slot_of, sizeof(int32_t) * (size_t)N));
+      G.slot_of = s->slot_of.as<int32_t>();
+    } else {
+      cg.nprim = any_rows ? (int)((N + CHUNK_T - 1) / CHUNK_T) : 0;
+      s->chunks_sparse = (cg.block[0] != 0 && s->Np > 0) || (cg.block[1] != 0 && N - s->Np > 0);
+      s->chunk_nprim = cg.nprim;
+      s->max_chunks = cg.nprim + overflow;
+      PASTA_TRY(buffer_reserve(s, &s->chunk_tab, sizeof(int32_t) * CHUNK_T * (size_t)(s->max_chunks + 8)));
+      PASTA_TRY(buffer_reserve(s, &s->chunk_first, sizeof(int32_t) * (size_t)N));
     }
-    for (int sp = 0; sp < 2; ++sp)
-      if (cg.block[sp] != 0 && (sp == 0 ? s->Np : N - s->Np) > 0) {
-        const int64_t nb = (s->grid_sp[sp].ncell + cg.block[sp] - 1) / cg.block[sp];
-        k1_chunk_blocks_kernel<<<grid_for(nb * nb * nb, 128), 128, 0, s->stream>>>(
-            sp, start, g, cg, s->chunk_tab.as<int32_t>(), n_overflow, s->chunk_first.as<int32_t>());
-        s->launches += 1;
-      }
+    k1_scatter_kernel<<<grid_for(N, B), B, 0, s->stream>>>(N, G.pbin, start, cnt, s->perm_raw.as<int32_t>(), n_overflow);
+    s->launches += 1;
+    if (!lists && any_rows) {
+      // gather + the DENSE builder's table entries in one launch
+      k1_gather_chunks_kernel<<<grid_for(N, GATHER_T), GATHER_T, 0, s->stream>>>(
+          G, (int32_t)s->Np, cg, s->chunk_tab.as<int32_t>(), n_overflow, s->chunk_first.as<int32_t>());
+    } else {
+      k1_gather_kernel<true><<<grid_for(N, B), B, 0, s->stream>>>(G);
+    }
+    s->launches += 1;
+    if (!lists) {
+      for (int sp = 0; sp < 2; ++sp)
+        if (cg.block[sp] != 0 && (sp == 0 ? s->Np : N - s->Np) > 0) {
+          const int64_t nb = (s->grid_sp[sp].ncell + cg.block[sp] - 1) / cg.block[sp];
+          k1_chunk_blocks_kernel<<<grid_for(nb * nb * nb, 128), 128, 0, s->stream>>>(
+              sp, start, g, cg, s->chunk_tab.as<int32_t>(), n_overflow, s->chunk_first.as<int32_t>());
+          s->launches += 1;
+        }
+    }
   }
   s->sort_kind = uniform ? 1 : (lists ? 2 : 0);
   PASTA_CUDA_OK(cudaGetLastError());
