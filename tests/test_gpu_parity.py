@@ -848,3 +848,27 @@ def test_steps_without_per_step_energies(N, Y_P, density, extra):
     a, b = out
     assert _torch().equal(a[0], b[0]) and _torch().equal(a[1], b[1])
     assert a[2] == b[2] and a[3] == b[3] and _torch().equal(a[4], b[4])
+
+
+def test_large_system_sampled_targets(orc):
+    """Eight times BASELINE config 4: 3 276 800 nucleons at n = 0.08 fm^-3 (L = 344.7 fm, 2.6e6 bins, 4.2e5 chunks) --
+    beyond every size the decompression runs reach at this density.  Forces and per-particle energies of 512 sampled
+    targets against the all-pairs oracle, the usual gates; properties that hold at any size; 3 MD steps."""
+    N = 8 * 409600
+    p = pasta.default_params(r_c=20.0, thermostat_interval=10)
+    with pasta.Sim(N, 0.3, 0.08, 0.5, params=p, seed=7) as sim:
+        x, v, is_p, L, _ = sim.get_state()
+        x, is_p = _np(x), _np(is_p)
+        F, pe = sim.forces()
+        F, e = _np(F), _np(sim.particle_energies())
+        t = np.sort(np.random.default_rng(5).choice(N, size=512, replace=False))
+        Fo, eo, _, d = orc.forces(x, is_p, L, _oparams(orc, p), targets=t)
+        _check_forces(F[t], Fo, alternates=_alts(orc, x, is_p, L, _oparams(orc, p), t), boundary_pairs=d["boundary_pairs"])
+        assert np.abs(e[t] - eo).max() <= 2e-6 * np.abs(eo).max() + 0.5 * 9.8e-3   # (+ one D22 flip of V_c(r_c) / 2)
+        assert e.sum() == pytest.approx(pe, rel=1e-12)
+        assert np.abs(F.sum(0)).max() <= 1e-6 * np.abs(F).sum()
+        pairs = sim.pair_count()
+        assert pairs == pytest.approx(N * 0.08 * 4.0 / 3.0 * math.pi * 20.0 ** 3, rel=2e-3)     # P12
+        sim.step(3, 2.0)
+        ke, _ = sim.energy()
+        assert math.isfinite(ke) and ke > 1.5 * N * 0.5   # (the overlapping nucleons of a random start heat it at once)
