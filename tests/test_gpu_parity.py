@@ -872,3 +872,43 @@ def test_large_system_sampled_targets(orc):
         sim.step(3, 2.0)
         ke, _ = sim.energy()
         assert math.isfinite(ke) and ke > 1.5 * N * 0.5   # (the overlapping nucleons of a random start heat it at once)
+
+
+@pytest.mark.parametrize("seed", list(range(16)))
+def test_random_modes_and_short_trajectories(orc, seed):
+    """Seeded sweep over the MODES: contract pair set, the paper's radial range split (r_nuc), its Coulomb sum without a
+    cut-off (boxes of >= 120 fm only, D26), with a fixed or scaling box, thermostat on or off -- sizes and densities
+    from dilute (reused neighbour lists) to dense (chunk kernel).  Forces and PE against the oracle run in the same
+    mode, then 4 steps of the trajectory against the oracle's integrator."""
+    rng = np.random.default_rng(5000 + seed)
+    N = int(rng.integers(200, 3000))
+    Y_P = float(rng.choice([0.05, 0.3, 0.5]))
+    mode = int(rng.integers(0, 3))
+    density = float(10 ** rng.uniform(-3.6, -2.9)) if mode == 2 else float(10 ** rng.uniform(-3.3, -1.1))
+    L = inputs.box_length(N, density)
+    if mode == 2 and L < 120.0:
+        mode = 1
+    r_c = float(min(20.0, 0.499 * L))
+    prm = dict(r_c=r_c)
+    okw = dict(r_c=r_c)
+    if mode >= 1 and r_c > 11.5:
+        prm["r_nuc"], okw["r_nuc"] = 11.5, 11.5
+    if mode == 2:
+        prm["coulomb_all_pairs"], okw["coul_nocut"] = 1, 1.0
+    scale = float(rng.choice([1.0, 1.0005]))
+    interval = int(rng.choice([0, 2]))
+    T = 0.5
+    x, v, is_p, L = inputs.uniform_state(N, Y_P, density, T, seed=seed)
+    op = orc.Params(**okw)
+    with _sim_from_arrays(x, v, is_p, L, T=T, scale_per_step=scale, thermostat_interval=interval, **prm) as sim:
+        F, pe = sim.forces()
+        Fo, _, peo, d = orc.forces(x, is_p, L, op)
+        alts = None if mode == 2 else _alts(orc, x, is_p, L, op)
+        _check_forces(_np(F), Fo, pe, peo if abs(peo) > 1e-9 else None, alts, d["boundary_pairs"])
+        sim.step(4, 2.0)
+        xg, _, _, Lg, _ = sim.get_state()
+        xo, vo, Lo, *_ = orc.step(x, v, is_p, L, op, T, interval, scale, 2.0, 4)
+        assert Lg == pytest.approx(Lo, rel=1e-14)
+        dd = _np(xg) - xo
+        dd -= Lo * np.round(dd / Lo)
+        assert np.quantile(np.linalg.norm(dd, axis=1), 0.99) <= TRAJ_TOL
