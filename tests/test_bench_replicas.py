@@ -43,3 +43,22 @@ def test_replica_aggregation_world_size_2(tmp_path):
     d = json.loads(line)
     assert d["dev_s"] == 2.0 and d["e2e_s"] == 4.0          # max over the two ranks
     assert d["value"] == 2 * 10 / 2.0                        # whole-job steps/s: all replicas' steps / slowest rank
+
+
+def test_bench_roofline_inputs_come_from_committed_files():
+    """bench.py's roofline arithmetic: 17 + 8 Y_P^2 FP32 and 1 + 2 Y_P^2 MUFU per ordered in-range pair,
+    and `traffic` read from the committed ncu summary of this round, never a literal."""
+    sys.path.insert(0, ROOT)
+    import bench
+
+    fp32, mufu = bench.algorithmic_cost(0.30)
+    assert abs(fp32 - 17.72) < 1e-9 and abs(mufu - 1.18) < 1e-9
+    traffic, src = bench.ncu_traffic(4)
+    assert traffic is not None and 5e6 < traffic < 5e7 and os.path.exists(os.path.join(ROOT, src))
+    text = open(os.path.join(ROOT, src)).read()
+    assert "ncu --set full" in text and "k2_chunk_kernel" in text
+    none, why = bench.ncu_traffic(2)
+    assert none is None and "no committed" in why
+    cfg = bench.workload_config(4, 1)
+    assert cfg["N"] == 409600 and "workload" in cfg and "model" not in cfg
+    assert "sharded" in bench.workload_config(4, 8, True)["parallelism"]
