@@ -78,6 +78,46 @@ __global__ void __launch_bounds__(1024) k_step(float* out, long long* cyc, float
   if (threadIdx.x == 0) cyc[blockIdx.x] = t1 - t0;
 }
 
+// Do other pipes' instructions issue in the shadow of packed FP32?  16 independent 2-operand FFMA2 per trip (32 pipe
+// cycles) interleaved with M integer ALU instructions (LOP3, 8 independent chains) or M shared-memory loads: if a packed
+// instruction kept only the FMA pipe for its second cycle the trip would cost max(32, 16 + M) cycles; if it keeps the
+// DISPATCH port it costs 32 + M.
+template <int M, bool LOADS>
+__global__ void __launch_bounds__(1024) k_mix(float* out, long long* cyc, float seed) {
+  __shared__ int sm[1024];
+  float2 p[8], q[8];
+  unsigned x[8];
+#pragma unroll
+  for (int i = 0; i < 8; ++i) { p[i] = make_float2(seed + i, seed - i); q[i] = make_float2(seed * i, seed + 2 * i + threadIdx.x); x[i] = threadIdx.x * 2654435761u + i; }
+  sm[threadIdx.x] = threadIdx.x;
+  __syncthreads();
+  const unsigned key = (unsigned)__float_as_int(seed) | 1u;
+  const unsigned a0 = (unsigned)__cvta_generic_to_shared(&sm[threadIdx.x & ~31]);
+  const long long t0 = clock64();
+#pragma unroll 1
+  for (int it = 0; it < ITERS; ++it) {
+#pragma unroll
+    for (int r = 0; r < 2; ++r) {
+#pragma unroll
+      for (int i = 0; i < 8; ++i) {
+        p[i] = __ffma2_rn(q[i], q[i], p[i]);
+#pragma unroll
+        for (int m = 0; m < (M >= 16 ? M / 16 : ((i + 8 * r) % (16 / (M > 0 ? M : 16)) == 0 && M > 0 ? 1 : 0)); ++m) {
+          if (LOADS) { int v; asm volatile("ld.shared.b32 %0, [%1];" : "=r"(v) : "r"(a0 + 4 * ((i + m + r) & 31)) : "memory"); x[i] ^= (unsigned)v; }
+          else if ((m + r) & 1) asm volatile("add.u32 %0, %0, %1;" : "+r"(x[i]) : "r"(key));   // (xor / add alternate: nothing to fold)
+          else asm volatile("xor.b32 %0, %0, %1;" : "+r"(x[i]) : "r"(key));
+        }
+      }
+    }
+  }
+  const long long t1 = clock64();
+  float s = 0;
+#pragma unroll
+  for (int i = 0; i < 8; ++i) s += p[i].x + p[i].y + q[i].x + (float)x[i];
+  out[blockIdx.x * blockDim.x + threadIdx.x] = s;
+  if (threadIdx.x == 0) cyc[blockIdx.x] = t1 - t0;
+}
+
 static float* g_out; static long long* g_cyc; static int g_sms;
 template <class F> static void run(const char* name, int w, double per_trip, F launch) {
   launch(w); launch(w);
@@ -100,6 +140,16 @@ int main() {
     run("fadd2_bcast", w, 32, [](int w_) { k_ops<4><<<g_sms, 128 * w_>>>(g_out, g_cyc, 1.0001f); });
     run("fmul2", w, 32, [](int w_) { k_ops<5><<<g_sms, 128 * w_>>>(g_out, g_cyc, 1.0001f); });
     run("eval_step", w, 4, [](int w_) { k_step<<<g_sms, 128 * w_>>>(g_out, g_cyc, 1.0001f); });
+    // SMSP-cycles per TRIP of 16 packed FFMA2 + M other instructions
+    run("mix16_alu0", w, 1, [](int w_) { k_mix<0, false><<<g_sms, 128 * w_>>>(g_out, g_cyc, 1.0001f); });
+    run("mix16_alu4", w, 1, [](int w_) { k_mix<4, false><<<g_sms, 128 * w_>>>(g_out, g_cyc, 1.0001f); });
+    run("mix16_alu8", w, 1, [](int w_) { k_mix<8, false><<<g_sms, 128 * w_>>>(g_out, g_cyc, 1.0001f); });
+    run("mix16_lds4", w, 1, [](int w_) { k_mix<4, true><<<g_sms, 128 * w_>>>(g_out, g_cyc, 1.0001f); });
+    run("mix16_lds8", w, 1, [](int w_) { k_mix<8, true><<<g_sms, 128 * w_>>>(g_out, g_cyc, 1.0001f); });
+    run("mix16_alu16", w, 1, [](int w_) { k_mix<16, false><<<g_sms, 128 * w_>>>(g_out, g_cyc, 1.0001f); });
+    run("mix16_alu32", w, 1, [](int w_) { k_mix<32, false><<<g_sms, 128 * w_>>>(g_out, g_cyc, 1.0001f); });
+    run("mix16_alu64", w, 1, [](int w_) { k_mix<64, false><<<g_sms, 128 * w_>>>(g_out, g_cyc, 1.0001f); });
+    run("mix16_lds16", w, 1, [](int w_) { k_mix<16, true><<<g_sms, 128 * w_>>>(g_out, g_cyc, 1.0001f); });
   }
   return 0;
 }
