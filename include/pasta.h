@@ -127,7 +127,9 @@ int pasta_forces(pasta_sim* sim, double* F_dev, double* pe_host);
  *   v += (dt/2M) F;  step count += 1;  if interval > 0 and count % interval == 0 and KE > 0:
  *   v *= sqrt(1.5 N T / KE)   (D7, D8).
  * Forces are evaluated first if they are stale (after create / set_state without forces / expand).
- * Asynchronous.  EINVAL: n < 0, dt <= 0, or the box would shrink below 2 r_c.
+ * Asynchronous -- except in the neighbour-list regime (list_reuse), where every step reads one word back from the device
+ * (the displacement trigger) while its force kernel runs.  On the chunk path a fixed-box step is replayed
+ * as a CUDA graph (pasta_graph_replays).  EINVAL: n < 0, dt <= 0, or the box would shrink below 2 r_c.
  */
 int pasta_step(pasta_sim* sim, int64_t n, double dt);
 
