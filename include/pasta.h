@@ -160,6 +160,46 @@ int pasta_cluster_sizes(pasta_sim* sim, int32_t* A_dev, int32_t* Z_dev);
  * A >= a_min, mean A, sigma A, mean Z, sigma Z over those clusters}.  Synchronises. */
 int pasta_composition(pasta_sim* sim, int32_t a_min, double* out6_host);
 
+/*
+ * Friends-of-friends labels WITHOUT any device allocation -- for callers that cannot get device memory at the moment
+ * they need cluster labels.  Two kinds of caller are meant: a process in which another component (a framework's
+ * caching allocator, a second library, a job sized to fill the 180 GB) already owns the device's free memory, so that
+ * cudaMalloc fails or would have to take memory away from it; and a caller running the analysis beside a simulation
+ * that is stepping on other streams, for which the device-wide synchronisation hidden in cudaMalloc / cudaFree would
+ * stall those steps.  pasta_clusters reserves up to seven internal arrays through pasta_env.alloc on its first call; this
+ * entry point needs no pasta_sim, calls neither cudaMalloc nor cudaFree nor any library routine that allocates, and
+ * enqueues only kernels and one 8-byte device-to-device copy on `stream`.  It returns without synchronising.
+ *
+ * What it computes is pasta_clusters' result (BASELINE variant of PAPER.md:154-158; D13): label_dev[i] = smallest
+ * particle index in the connected component of i in the graph {(i, j): r_ij <= r_cl} at the nearest image, the same
+ * pinned FP64 predicate, so the labels are identical bit for bit.  (A, Z) histograms and the MST variant are not
+ * offered here.
+ *   x_dev [N][3]      positions on `device`, as pasta_get_state returns them (input, read only)
+ *   label_dev [N]     output, on `device`
+ *   n_clusters_dev    output, ONE int64 on `device` (not a host pointer: a host scalar would force a synchronisation);
+ *                     may be NULL
+ *   device, stream    the CUDA device that holds the buffers -- the call makes it current and leaves it current, as
+ *                     every other entry point of this library does -- and a cudaStream_t of it (NULL = default stream)
+ *
+ * The price is a fixed ceiling.  The union-find forest lives in a static device array inside the library image,
+ * PASTA_CLUSTERS_NOALLOC_MAX_N entries (256 KiB), which every GPU that loads the library carries until the process
+ * ends.  N above the ceiling is refused with PASTA_EINVAL and a message that names it; nothing is enqueued then.
+ * Candidate pairs are enumerated all against all (no cell list, which would need four more scratch arrays): the cost
+ * is N^2/2 FP64 predicates, so it is slower than pasta_clusters, whose cell list makes the work linear in N.
+ *
+ * Set-up: the first call on each device looks up the device address of that array (cudaGetSymbolAddress, which also
+ * loads the module on that device).  Make that first call outside any stream capture; later calls on the same device
+ * do no set-up.
+ * Sharing: all calls on one GPU use the SAME array.  Each call re-initialises the part it uses, so stale contents of
+ * an earlier call never leak into a result -- but two calls whose kernels may run at the same time on one GPU (two
+ * streams, two host threads) race on it and both results are then garbage.  Order them on one stream or with events.
+ * EINVAL: N < 0 or N > PASTA_CLUSTERS_NOALLOC_MAX_N; x_dev or label_dev NULL with N > 0; L <= 0; r_cl <= 0 or
+ * r_cl > L/2; device outside [0, 64).  N == 0 is allowed (writes 0 to n_clusters_dev).
+ */
+#define PASTA_CLUSTERS_NOALLOC_MAX_N 65536
+int pasta_clusters_noalloc(const double* x_dev, int64_t N, double L, double r_cl, int32_t* label_dev,
+                           int64_t* n_clusters_dev, int32_t device, void* stream);
+
 /* State accessors.  Any pointer may be NULL (skipped).  get_* with a host scalar synchronises. */
 int pasta_get_state(pasta_sim* sim, double* x_dev, double* v_dev, uint8_t* is_proton_dev, double* L_host,
                     int64_t* step_host);

@@ -4,4 +4,5 @@
 workloads.  Importing this package loads neither torch nor the CUDA library.
 """
 from . import inputs  # noqa: F401
-from .binding import Env, Params, PastaError, Sim, default_params, library_path, load, shard_bounds  # noqa: F401
+from .binding import (CLUSTERS_NOALLOC_MAX_N, Env, Params, PastaError, Sim, clusters_noalloc,  # noqa: F401
+                      default_params, library_path, load, shard_bounds)

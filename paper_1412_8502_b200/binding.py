@@ -55,6 +55,8 @@ SIGNATURES = {
     "pasta_expand": (C.c_int, [C.c_void_p, C.c_double]),
     "pasta_clusters": (C.c_int, [C.c_void_p, C.c_double, C.c_void_p, C.POINTER(C.c_int64)]),
     "pasta_clusters_mst": (C.c_int, [C.c_void_p, C.c_double, C.c_double, C.c_void_p, C.POINTER(C.c_int64)]),
+    "pasta_clusters_noalloc": (C.c_int, [C.c_void_p, C.c_int64, C.c_double, C.c_double, C.c_void_p, C.c_void_p,
+                                         C.c_int32, C.c_void_p]),
     "pasta_cluster_sizes": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p]),
     "pasta_composition": (C.c_int, [C.c_void_p, C.c_int32, C.POINTER(C.c_double)]),
     "pasta_get_state": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.POINTER(C.c_double),
@@ -117,6 +119,37 @@ def shard_bounds(N, Np, cost_p, cost_n, world):
     out = (C.c_int64 * (int(world) + 1))()
     _check(load().pasta_shard_bounds(int(N), int(Np), float(cost_p), float(cost_n), int(world), out))
     return [int(b) for b in out]
+
+
+CLUSTERS_NOALLOC_MAX_N = 65536  # PASTA_CLUSTERS_NOALLOC_MAX_N of include/pasta.h
+
+
+def clusters_noalloc(x, L, r_cl, label_out, n_clusters_out=None, stream=None):
+    """pasta_clusters_noalloc: friends-of-friends labels of the positions x ([N,3] float64 cuda tensor, box side L)
+    written into label_out ([N] int32 cuda) and the number of clusters into n_clusters_out ([1] int64 cuda, optional).
+
+    For callers that cannot allocate device memory when they need the labels -- the free memory of the GPU belongs to
+    someone else's pool, or a cudaMalloc would stall a simulation stepping on other streams.  Neither this wrapper nor
+    the library call behind it allocates on the device: the outputs are the caller's tensors and the working memory is
+    a fixed array inside the library, which limits N to CLUSTERS_NOALLOC_MAX_N (a larger N raises PastaError, code -1).
+    Nothing is synchronised; the results are ordered with `stream` (default: torch's current stream of x's device).
+    All calls on one GPU share that working array: do not let two of them overlap on the device."""
+    import torch
+
+    if not (x.is_cuda and x.dtype == torch.float64 and x.is_contiguous() and x.dim() == 2 and x.shape[1] == 3):
+        raise ValueError("x must be a contiguous [N,3] float64 cuda tensor")
+    N = x.shape[0]
+    if not (label_out.is_cuda and label_out.dtype == torch.int32 and label_out.is_contiguous()
+            and label_out.numel() == N and label_out.device == x.device):
+        raise ValueError("label_out must be a contiguous [N] int32 tensor on x's device")
+    if n_clusters_out is not None and not (n_clusters_out.dtype == torch.int64 and n_clusters_out.numel() == 1
+                                           and n_clusters_out.device == x.device):
+        raise ValueError("n_clusters_out must be one int64 on x's device")
+    st = torch.cuda.current_stream(x.device) if stream is None else stream
+    _check(load().pasta_clusters_noalloc(
+        C.c_void_p(x.data_ptr()), N, float(L), float(r_cl), C.c_void_p(label_out.data_ptr()),
+        None if n_clusters_out is None else C.c_void_p(n_clusters_out.data_ptr()), x.device.index,
+        C.c_void_p(st.cuda_stream)))
 
 
 def default_params(**overrides):

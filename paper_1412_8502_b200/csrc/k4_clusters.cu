@@ -6,6 +6,8 @@
 // canonical labels (smallest member index) -- is identical to a brute-force FP64 enumeration.
 // Candidates come from a cell grid of width >= r_cl (own + 26 neighbour cells).  Roots are always the
 // smaller index (hook larger root under smaller with atomicCAS), so after flattening label = min index.
+#include <mutex>
+
 #include "pasta_internal.cuh"
 
 namespace pasta {
@@ -302,3 +304,103 @@ int k4_composition(Sim* s, int32_t a_min, double* out6_host) {
 }
 
 }  // namespace pasta
+
+// -----------------------------------------------------------------------------------------------------------------
+// pasta_clusters_noalloc -- friends-of-friends labels for callers that must not allocate device memory (pasta.h).
+//
+// Same edges, same predicate, same canonical labels as k4_clusters with r_np == 0; what differs is where the working
+// memory lives.  k4_clusters takes its union-find forest (and cell lists) from the simulation's allocator.  Here the
+// forest sits in the file-scope array below, which is part of the library image: every GPU on which this module gets
+// loaded carries these PASTA_CLUSTERS_NOALLOC_MAX_N * 4 + 256 bytes until the process exits, whether the entry point
+// is ever called or not.  That is why the maximum is modest, and why the link step is the all-pairs kernel (it needs
+// the forest and nothing else; the cell-list variant would need four more arrays of scratch).
+//
+//   noalloc_scratch[0 .. MAX_N)   parent[] of the union-find forest
+//   noalloc_scratch[MAX_N, +2)    the root counter (one unsigned 64-bit word, 8-byte aligned since MAX_N * 4 % 256 == 0)
+//
+// The array keeps whatever the previous call left in it, so every call re-initialises the part it uses (parent[i] = i
+// for i < N, counter = 0) on the caller's stream before linking.  There is ONE array per GPU: two calls whose kernels
+// can overlap on the same GPU (different streams, different host threads) corrupt each other's forest.
+// -----------------------------------------------------------------------------------------------------------------
+static_assert((PASTA_CLUSTERS_NOALLOC_MAX_N * 4) % 256 == 0, "the root counter must stay 8-byte aligned");
+static __device__ __align__(256) int32_t noalloc_scratch[PASTA_CLUSTERS_NOALLOC_MAX_N + 64];
+
+namespace pasta {
+
+__global__ void k4_noalloc_init_kernel(int64_t N, int32_t* __restrict__ parent, unsigned long long* __restrict__ n_roots) {
+  int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i == 0) *n_roots = 0ull;
+  if (i < N) parent[i] = (int32_t)i;
+}
+
+// The flatten step of k4_flatten_kernel without the (A, Z) histograms, which would be two more scratch arrays.
+__global__ void k4_noalloc_labels_kernel(int64_t N, int32_t* __restrict__ parent, int32_t* __restrict__ label_out,
+                                         unsigned long long* __restrict__ n_roots) {
+  int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= N) return;
+  const int r = uf_find(parent, (int)i);
+  label_out[i] = r;
+  if (r == (int)i) atomicAdd(n_roots, 1ull);
+}
+
+// `noalloc_scratch` in HOST code is only a handle for the runtime, not a device address.  The address a kernel can
+// use is per device and is asked for once per device, with that device current; it is cached here afterwards.
+static const int kNoAllocMaxDevices = 64;
+static std::mutex noalloc_mutex;
+static int32_t* noalloc_ptr[kNoAllocMaxDevices] = {};
+
+static int noalloc_scratch_on(int device, int32_t** out) {  // `device` is current
+  std::lock_guard<std::mutex> lock(noalloc_mutex);
+  if (!noalloc_ptr[device]) {
+    void* p = nullptr;
+    PASTA_CUDA_OK(cudaGetSymbolAddress(&p, noalloc_scratch));
+    if (!p) {
+      set_error("pasta_clusters_noalloc: cudaGetSymbolAddress returned a null scratch address on device %d", device);
+      return PASTA_ECUDA;
+    }
+    noalloc_ptr[device] = static_cast<int32_t*>(p);
+  }
+  *out = noalloc_ptr[device];
+  return PASTA_OK;
+}
+
+}  // namespace pasta
+
+int pasta_clusters_noalloc(const double* x_dev, int64_t N, double L, double r_cl, int32_t* label_dev,
+                           int64_t* n_clusters_dev, int32_t device, void* stream) {
+  using namespace pasta;
+  // every argument is checked before the first CUDA call
+  if (N < 0 || N > (int64_t)PASTA_CLUSTERS_NOALLOC_MAX_N) {
+    set_error("pasta_clusters_noalloc: N = %lld is outside [0, %d]: the scratch memory of this entry point is a fixed "
+              "array of PASTA_CLUSTERS_NOALLOC_MAX_N entries; larger systems need pasta_clusters, which allocates",
+              (long long)N, (int)PASTA_CLUSTERS_NOALLOC_MAX_N);
+    return PASTA_EINVAL;
+  }
+  if (N > 0 && (!x_dev || !label_dev)) {
+    set_error("pasta_clusters_noalloc: x_dev and label_dev must not be NULL");
+    return PASTA_EINVAL;
+  }
+  if (!(L > 0.0) || !(r_cl > 0.0) || r_cl > 0.5 * L) {
+    set_error("pasta_clusters_noalloc: need L > 0 and 0 < r_cl <= L/2");
+    return PASTA_EINVAL;
+  }
+  if (device < 0 || device >= kNoAllocMaxDevices) {
+    set_error("pasta_clusters_noalloc: device ordinal %d is outside [0, %d)", (int)device, kNoAllocMaxDevices);
+    return PASTA_EINVAL;
+  }
+  PASTA_CUDA_OK(cudaSetDevice(device));
+  int32_t* parent = nullptr;
+  PASTA_TRY(noalloc_scratch_on(device, &parent));
+  unsigned long long* n_roots = reinterpret_cast<unsigned long long*>(parent + PASTA_CLUSTERS_NOALLOC_MAX_N);
+  cudaStream_t st = static_cast<cudaStream_t>(stream);
+  const int B = 256;
+  k4_noalloc_init_kernel<<<grid_for(N > 0 ? N : 1, B), B, 0, st>>>(N, parent, n_roots);
+  if (N > 0) {
+    k4_link_all_kernel<<<grid_for(N, 128), 128, 0, st>>>(N, x_dev, L, 1.0 / L, r_cl * r_cl, parent, nullptr);
+    k4_noalloc_labels_kernel<<<grid_for(N, B), B, 0, st>>>(N, parent, label_dev, n_roots);
+  }
+  PASTA_CUDA_OK(cudaGetLastError());
+  if (n_clusters_dev)
+    PASTA_CUDA_OK(cudaMemcpyAsync(n_clusters_dev, n_roots, sizeof(int64_t), cudaMemcpyDeviceToDevice, st));
+  return PASTA_OK;
+}
