@@ -220,7 +220,9 @@ int pasta_set_state_host(pasta_sim* sim, const double* x_host, const double* v_h
  * already crossing PCIe in one direction and the result of step k - 1 in the other.  Both calls return at once.
  *   pasta_set_state_host_async: x, v, F (F may be NULL: forces stale) are copied host -> staging on the upload stream;
  *     the simulation's stream then takes them over (device copy, wrap into [0, L)).  The host buffers may be reused
- *     after the NEXT BUT ONE async set, or after pasta_host_sync.
+ *     after the NEXT BUT ONE async set has returned, or after pasta_host_sync: from the third call on, a call first
+ *     waits ON THE HOST until the copies of the set before last have left their host buffers (normally long done; it
+ *     blocks only a host that has run more than two uploads ahead of the device).
  *   pasta_get_state_host_async: the simulation's stream snapshots x, v, F into staging (forces evaluated first if
  *     stale); the download stream copies the snapshot to the host buffers, which are valid after pasta_host_sync (or
  *     after the next but one async get has returned and been synchronised).  L and the step count are returned at once
@@ -272,7 +274,10 @@ int pasta_pair_counts(pasta_sim* sim, int64_t* out2_host);
 
 /* Work statistics of one evaluation with the chunk pair kernel: out3_host = {sources streamed from the cell
  * rows (summed over chunks), tiles of <= 32 sources, pair evaluations executed}.  Synchronises.
- * (ordered in-range pairs / pair evaluations = the kernel's useful-work fraction.) */
+ * (ordered in-range pairs / pair evaluations = the kernel's useful-work fraction.)  The evaluation covers every
+ * target even under pasta_set_shard (no collective is issued; every rank computes the same complete F).  Its forces
+ * are kept for the next pasta_step except with coulomb_all_pairs, where the chunk kernel's F lacks the Coulomb term
+ * and the next consumer evaluates again. */
 int pasta_force_stats(pasta_sim* sim, int64_t* out3_host);
 /* Neighbour-list bookkeeping (list_reuse): out2_host = {force evaluations so far, of which rebuilt the list}. */
 int pasta_list_stats(pasta_sim* sim, int64_t* out2_host);

@@ -693,6 +693,7 @@ int k1_export_cells(Sim* s, int32_t* cell_id_dev, int32_t* cell_start_dev) {
   s->hist_valid = false;  // cell_id and the histogram table are about to hold the exported grid
   s->bins_zeroed = 0;
   s->sort_kind = -1;
+  s->list.valid = false;  // reused neighbour lists go with the sort they were built on (their consumers check sort_kind)
   PASTA_TRY(buffer_reserve(s, &s->bin_count, sizeof(int32_t) * (size_t)(g.nc3 + 1)));
   PASTA_TRY(buffer_reserve(s, &s->bin_start, sizeof(int32_t) * (size_t)(g.nc3 + 1)));
   int32_t* cnt = s->bin_count.as<int32_t>();

@@ -45,8 +45,11 @@ int buffer_reserve(Sim* s, Buffer* b, size_t bytes) {
 
 void buffer_release(Sim* s, Buffer* b) {
   if (!b->ptr) return;
-  // pending work on the stream may still use the buffer
-  cudaStreamSynchronize(s->stream);
+  // pending work on the stream may still use the buffer.  While a step is being captured s->stream is the capture
+  // stream: synchronising it is illegal (it would invalidate the capture) and it carries no pending work anyway --
+  // the kernels of the previous steps are on the caller's stream.  (A buffer that moves bumps state_gen, so the
+  // capture under way is discarded and the step redone kernel by kernel.)
+  cudaStreamSynchronize(s->graph.capturing ? s->graph.home : s->stream);
   if (s->env.alloc && s->env.free)
     s->env.free(b->ptr, s->env.user);
   else if (!s->env.alloc)
@@ -178,8 +181,8 @@ static int evaluate_forces(Sim* s, bool with_energy, double kick = 0.0) {
       if (lists) {
         const double halo = list_halo(s);
         const int rc = k2_list_build(s, halo);
-        if (rc == 1) {  // too dense for lists after all (a clustered state): the chunk kernel on its own sort, from now on
-          s->no_lists = true;
+        if (rc == 1) {  // too dense for lists after all (a clustered state): the chunk kernel on its own sort, until the
+          s->no_lists = true;  // caller brings another state or box (pasta_set_state*, pasta_expand try lists again)
           PASTA_TRY(k1_build(s));
           return evaluate_forces_tail(s, with_energy);
         }
@@ -325,9 +328,12 @@ static int step_once(Sim* s, double dt, double sc, double L_wrap, bool energy, b
       return step_body(s, dt, sc, L_wrap, energy, rescale);
     }
     cudaStream_t const user_stream = s->stream;
+    s->graph.home = user_stream;
+    s->graph.capturing = true;
     s->stream = s->graph.cap;
     const int rc = step_body(s, dt, sc, L_wrap, energy, rescale);
     s->stream = user_stream;
+    s->graph.capturing = false;
     cudaGraph_t g = nullptr;
     const cudaError_t ce = cudaStreamEndCapture(s->graph.cap, &g);
     if (rc != PASTA_OK || ce != cudaSuccess || !g || s->graph.gen != s->state_gen) {
@@ -613,6 +619,7 @@ int pasta_expand(pasta_sim* sim, double scale) {
   const double L_new = s->L * scale;
   PASTA_TRY(k3_wrap_scale(s, scale, L_new));
   s->list.valid = false;
+  s->no_lists = false;  // another box: lists get another try
   s->L = L_new;
   s->lin_L0 = L_new;
   s->lin_n = 0;
@@ -689,6 +696,7 @@ int pasta_get_state(pasta_sim* sim, double* x_dev, double* v_dev, uint8_t* is_pr
 
 static int after_set_state(Sim* s, bool have_is_p, bool have_F, double L) {
   s->list.valid = false;
+  s->no_lists = false;  // a new configuration: it may be dilute where the last one was too dense for lists
   s->L = L;
   s->lin_L0 = L;
   s->lin_n = 0;
@@ -782,6 +790,10 @@ int pasta_set_state_host_async(pasta_sim* sim, const double* x_host, const doubl
   const int b = (int)(p.n_in & 1);
   const size_t n = 24 * (size_t)s->N;
   char* st = p.in[b].as<char>();
+  // The host buffers of the set before last may be refilled as soon as this call returns (pasta.h).  Its copies sit on
+  // the upload stream behind a wait for the simulation's stream, so they may not even have started: wait for them
+  // here, on the host.  (That set used this same slot b, and the pipeline stays two uploads deep.)
+  if (p.n_in >= 2) PASTA_CUDA_OK(cudaEventSynchronize(p.in_done[b]));
   // upload stream: the staging buffer is free once the simulation's stream has taken the upload before last
   if (p.n_in >= 2) PASTA_CUDA_OK(cudaStreamWaitEvent(p.up, p.in_taken[b], 0));
   PASTA_CUDA_OK(cudaMemcpyAsync(st, x_host, n, cudaMemcpyHostToDevice, p.up));
@@ -974,9 +986,15 @@ int pasta_force_stats(pasta_sim* sim, int64_t* out3_host) {
   int rc = k1_build(s);
   s->no_lists = no_lists;
   PASTA_TRY(rc);
+  // The statistics are those of ONE complete evaluation by the chunk kernel: every target, whatever window
+  // pasta_set_shard last left behind (a sharded evaluation recomputes its window each time).
+  s->shard.slot_lo = 0;
+  s->shard.slot_hi = 0x7fffffff;
   PASTA_TRY(k2_chunk_forces(s, true, true));
-  s->forces_valid = true;
-  s->energies_valid = true;
+  // F and e now hold every term the chunk kernel computes, for every particle, and on every rank alike: they ARE the
+  // forces of this configuration -- unless the Coulomb term comes from a kernel of its own (coulomb_all_pairs), which
+  // did not run: then they are a by-product that nobody may use, and the next consumer re-evaluates.
+  s->forces_valid = s->energies_valid = !s->prm.coulomb_all_pairs;
   unsigned long long h[3];
   PASTA_CUDA_OK(cudaMemcpyAsync(h, s->counters.as<unsigned long long>() + 10, sizeof(h), cudaMemcpyDeviceToHost,
                                 s->stream));

@@ -234,7 +234,8 @@ struct Sim {
   Buffer slot_of;     // int32[N] original index -> sorted slot (inverse of perm)
   Buffer list_off, list_pool;  // int4[N] {proton list: first, length; neutron list: first, length}; int32 sorted slots
   int64_t list_entries = 0;
-  bool no_lists = false;       // transient: the caller needs the chunk kernel's own sort (pasta_force_stats)
+  bool no_lists = false;       // lists are off: for one call (pasta_force_stats needs the chunk kernel's own sort), or since a
+                               // list build found the state too dense -- until the next set_state / expand, which retry
 
   // pair-force chunk table (k1_cells.cu -> k2_chunk.cu): [0, max_chunks) entries first slot | count << 26,
   // [max_chunks, 2 max_chunks) the list of chunks that need several rounds; the counters live in
@@ -263,6 +264,8 @@ struct Sim {
     int64_t gen = -1;              // value of state_gen at capture
     int64_t replays = 0;           // steps replayed so far
     cudaStream_t cap = nullptr;    // capture happens on a stream of our own (the caller's may be the legacy default stream)
+    bool capturing = false;        // s->stream is `cap` right now and must not be synchronised; the caller's stream is `home`
+    cudaStream_t home = nullptr;
     int warm = 0;                  // eligible steps enqueued kernel by kernel since the last change (buffers settle)
   } graph;
   // target sharding over several GPUs (pasta_set_shard): this rank evaluates the targets in sorted slots [slot_lo, slot_hi)
