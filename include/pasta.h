@@ -77,9 +77,17 @@ typedef struct pasta_params {
                                   every other proton"): the screened Coulomb term is summed over ALL proton pairs at their
                                   nearest image (a cube of side L, no radial cut-off; N_p^2 pair terms by a kernel of its
                                   own) and the nuclear terms stop at r_nuc, which must be set; r_c then only sizes the
-                                  cell list.  0 (default): the Coulomb term lives inside r_c like every other (D1) */
+                                  cell list.  0 (default): the Coulomb term lives inside r_c like every other (D1).
+                                  Needs a box side L >= PASTA_COULOMB_ALL_PAIRS_MIN_L (120 fm) at all times -- create,
+                                  set_state*, expand and a scaling step return PASTA_EINVAL below it.  Why: the image of
+                                  a pair is chosen on the FP32 leading parts of the box fractions x/L, so a pair within
+                                  6e-8 L of L/2 along an axis can take the other image, which changes its two forces by
+                                  2 F_c(L/2): 7e-6 MeV/fm at 120 fm (below the 1e-5 parity gate, and that is the range
+                                  the mode is verified in against the oracle), but 1e-3 at 55 fm (reading D26) */
   int32_t reserved1;
 } pasta_params;
+
+#define PASTA_COULOMB_ALL_PAIRS_MIN_L 120.0 /* fm; see pasta_params.coulomb_all_pairs */
 
 /* Device environment: where internal memory and the stream come from. */
 typedef void* (*pasta_alloc_fn)(size_t bytes, void* user); /* returns a device pointer (256-B aligned) or NULL */
@@ -105,7 +113,8 @@ int pasta_params_default(pasta_params* p);
  * with variance T/M (D15).  T is also the thermostat target.  env may be NULL (device 0,
  * default stream, cudaMalloc).
  * EINVAL: out/p NULL, wrong struct_size, N <= 0 or N >= 2^26 (sorted slots are packed in 26 bits), Y_P outside [0,1], density <= 0, T < 0,
- * r_c <= 0, r_c > L/2 (the nearest image would be ambiguous; D3), Lambda/lambda/mass <= 0,
+ * r_c <= 0, r_c > L/2 (the nearest image would be ambiguous; D3), coulomb_all_pairs with L < 120 fm,
+ * Lambda/lambda/mass <= 0,
  * scale_per_step <= 0, thermostat_interval < 0, cell_subdiv < 1.
  */
 int pasta_create(pasta_sim** out, int64_t N, double Y_P, double density, double T, const pasta_params* p,

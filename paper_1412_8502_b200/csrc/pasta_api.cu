@@ -415,6 +415,23 @@ int pasta_params_default(pasta_params* p) {
   return PASTA_OK;
 }
 
+// Smallest box side a parameter set may run in: 2 r_c (one nearest image within the cut-off; D3) and, with
+// coulomb_all_pairs, PASTA_COULOMB_ALL_PAIRS_MIN_L (pasta.h; D26).
+static double min_box_side(const pasta_params& p) {
+  const double two_rc = 2.0 * p.r_c;
+  return p.coulomb_all_pairs != 0 && two_rc < PASTA_COULOMB_ALL_PAIRS_MIN_L ? PASTA_COULOMB_ALL_PAIRS_MIN_L : two_rc;
+}
+static int check_box_side(const pasta_params& p, double L, const char* who) {
+  if (L > 0.0 && p.r_c <= 0.5 * L && L >= min_box_side(p)) return PASTA_OK;
+  if (L > 0.0 && p.r_c <= 0.5 * L)
+    set_error("%s: coulomb_all_pairs needs a box side of at least %g fm (got %g): the nearest image of a proton pair is "
+              "decided in FP32 box fractions, and the force error of a pair that lands on the wrong side of L/2 is "
+              "only negligible from there on (pasta.h)", who, (double)PASTA_COULOMB_ALL_PAIRS_MIN_L, L);
+  else
+    set_error("%s: need L >= 2 r_c (L = %g, r_c = %g): the nearest image would be ambiguous", who, L, p.r_c);
+  return PASTA_EINVAL;
+}
+
 static int validate_params(const pasta_params* p, double L) {
   if (!p || p->struct_size != sizeof(pasta_params)) {
     set_error("pasta_params is NULL or has the wrong struct_size");
@@ -442,7 +459,7 @@ static int validate_params(const pasta_params* p, double L) {
     set_error("r_c = %g exceeds L/2 = %g: the nearest image would be ambiguous", p->r_c, 0.5 * L);
     return PASTA_EINVAL;
   }
-  return PASTA_OK;
+  return check_box_side(*p, L, "pasta_create");
 }
 
 int pasta_create(pasta_sim** out, int64_t N, double Y_P, double density, double T, const pasta_params* p,
@@ -601,6 +618,7 @@ int pasta_step(pasta_sim* sim, int64_t n, double dt) {
       set_error("pasta_step: box side %g would fall below 2 r_c", L_new);
       return PASTA_EINVAL;
     }
+    PASTA_TRY(check_box_side(s->prm, L_new, "pasta_step"));
     s->L = L_new;
     const bool rescale = s->prm.thermostat_interval > 0 && ((s->step_count + 1) % s->prm.thermostat_interval) == 0;
     PASTA_TRY(step_once(s, dt, sc, linear ? L_old : L_new, energy, rescale));
@@ -615,6 +633,7 @@ int pasta_expand(pasta_sim* sim, double scale) {
     set_error("pasta_expand: need scale > 0 and scale*L >= 2 r_c");
     return PASTA_EINVAL;
   }
+  PASTA_TRY(check_box_side(s->prm, scale * s->L, "pasta_expand"));
   PASTA_TRY(use_device(s));
   const double L_new = s->L * scale;
   PASTA_TRY(k3_wrap_scale(s, scale, L_new));
@@ -719,6 +738,7 @@ int pasta_set_state(pasta_sim* sim, const double* x_dev, const double* v_dev, co
     set_error("pasta_set_state: need L >= 2 r_c");
     return PASTA_EINVAL;
   }
+  PASTA_TRY(check_box_side(s->prm, L, "pasta_set_state"));
   PASTA_TRY(use_device(s));
   const size_t n = (size_t)s->N;
   if (x_dev) PASTA_CUDA_OK(cudaMemcpyAsync(s->x.ptr, x_dev, 24 * n, cudaMemcpyDeviceToDevice, s->stream));
@@ -736,6 +756,7 @@ int pasta_set_state_host(pasta_sim* sim, const double* x_host, const double* v_h
     set_error("pasta_set_state_host: need L >= 2 r_c");
     return PASTA_EINVAL;
   }
+  PASTA_TRY(check_box_side(s->prm, L, "pasta_set_state_host"));
   PASTA_TRY(use_device(s));
   const size_t n = (size_t)s->N;
   if (x_host) PASTA_CUDA_OK(cudaMemcpyAsync(s->x.ptr, x_host, 24 * n, cudaMemcpyHostToDevice, s->stream));
@@ -784,6 +805,7 @@ int pasta_set_state_host_async(pasta_sim* sim, const double* x_host, const doubl
     set_error("pasta_set_state_host_async: need x, v and L >= 2 r_c");
     return PASTA_EINVAL;
   }
+  PASTA_TRY(check_box_side(s->prm, L, "pasta_set_state_host_async"));
   PASTA_TRY(use_device(s));
   PASTA_TRY(pipe_setup(s));
   Sim::HostPipe& p = s->pipe;

@@ -55,6 +55,9 @@ def test_argument_validation_happens_before_any_device_work():
         q = pasta.default_params()
         setattr(q, field, val)
         assert lib.pasta_create(C.byref(h), 51200, 0.4, 0.08, 1.0, C.byref(q), 1, None) == -1
+    q = pasta.default_params(r_nuc=11.5, coulomb_all_pairs=1)  # the paper's Coulomb sum needs a 120 fm box (D26); L = 86 fm here
+    assert lib.pasta_create(C.byref(h), 51200, 0.4, 0.08, 1.0, C.byref(q), 1, None) == -1
+    assert b"120" in lib.pasta_last_error()
     assert lib.pasta_create(None, 51200, 0.4, 0.08, 1.0, C.byref(p), 1, None) == -1
     assert lib.pasta_step(None, 1, 2.0) == -1 and lib.pasta_destroy(None) == 0
     assert lib.pasta_launch_count(None) == 0

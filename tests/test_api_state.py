@@ -101,7 +101,7 @@ def test_cells_then_step_on_reused_lists_with_coulomb_all_pairs():
     prm = dict(r_c=20.0, r_nuc=11.5, coulomb_all_pairs=1)
     res = []
     for detour in (False, True):
-        with pasta.Sim(5000, 0.4, 0.003, 0.5, seed=3, params=pasta.default_params(**prm)) as sim:
+        with pasta.Sim(5000, 0.4, 0.0028, 0.5, seed=3, params=pasta.default_params(**prm)) as sim:
             sim.step(4, 2.0)
             st = sim.list_stats()
             assert st["list_builds"] < st["force_evals"]  # the neighbour-list regime, lists being reused

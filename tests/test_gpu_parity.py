@@ -232,7 +232,8 @@ def test_config1_trajectory_20_steps(orc, seed):
     The uniform-random start has overlapping nucleons and is chaotic: the oracle's own 20-step response to
     a 1e-7 fm perturbation of the initial positions (one FP32 ulp of a cell-relative coordinate) is
     1.2e-4 .. 3e-4 fm at the worst particle (reading D19).  So the gate is: 99 % of the
-    particles within 1e-4 fm (median within 1e-5), and the worst particle within 3x max(1e-4 fm, that response)."""
+    particles within 1e-4 fm (median within 1e-5), and the worst particle within max(1e-4 fm, that response) --
+    1x, not a multiple of it: the measured worst particle is below the response on every seed (profiles/r2_results.md)."""
     c = inputs.CONFIGS[1]
     p = pasta.default_params(r_c=c["r_c"], thermostat_interval=0)
     op = _oparams(orc, p)
@@ -257,7 +258,7 @@ def test_config1_trajectory_20_steps(orc, seed):
                      "max": float(err.max()), "oracle_response_1e-7_max": float(intrinsic.max()),
                      "oracle_response_1e-7_q99": float(np.quantile(intrinsic, 0.99))})
         assert np.quantile(err, 0.99) <= TRAJ_TOL
-        assert err.max() <= 3 * max(TRAJ_TOL, intrinsic.max()), "trajectory error %.3e fm" % err.max()
+        assert err.max() <= max(TRAJ_TOL, intrinsic.max()), "trajectory error %.3e fm" % err.max()
         assert np.median(err) <= 0.1 * TRAJ_TOL
         assert np.abs(_np(vg) - vo).max() * c["dt"] <= 3 * max(TRAJ_TOL, intrinsic.max())
         ke, pe = sim.energy()
@@ -474,8 +475,9 @@ def test_forces_are_reproducible_run_to_run():
 def test_full_size_configs(orc, cfg):
     """BASELINE configs 2 and 4 at full size, in bench.py's launch configuration.  Config 2 (51 200) is compared in
     FULL: every force, every per-particle energy and the total PE against the all-pairs oracle.  Config 4 (409 600) on
-    4 096 sampled targets one by one (forces, energies, their PE sum at the 1e-6 gate), plus properties that hold
-    at any size."""
+    4 096 sampled targets one by one (forces, energies, their PE sum at the 1e-6 gate), the TOTAL PE of all 409 600
+    against the oracle's 27-cell evaluation of the same state at the 1e-6 gate (its forces too, as a relative L2 norm),
+    plus properties that hold at any size."""
     c = inputs.CONFIGS[cfg]
     p = pasta.default_params(r_c=c["r_c"], thermostat_interval=c["thermostat_interval"])
     with pasta.Sim(c["N"], c["Y_P"], c["density"], c["T"], params=p, seed=1) as sim:
@@ -490,6 +492,10 @@ def test_full_size_configs(orc, cfg):
         else:
             t = np.sort(np.random.default_rng(cfg).choice(c["N"], size=4096, replace=False))
             Fo, eo, _, d = orc.forces(x, is_p, L, _oparams(orc, p), targets=t)
+            Fc, ec, pec, _ = orc.forces_cells(x, is_p, L, _oparams(orc, p))   # every particle (orc_forces_cells is
+            assert abs(pe - pec) <= PE_TOL * abs(pec), "total PE %r vs %r" % (pe, pec)  # pinned to orc_forces: P7)
+            assert np.linalg.norm(F - Fc) / np.linalg.norm(Fc) <= FORCE_TOL
+            assert np.array_equal(Fc[t], Fo) or np.abs(Fc[t] - Fo).max() <= 1e-12 * np.abs(Fo).max()
         _check_forces(F[t], Fo, alternates=_alts(orc, x, is_p, L, _oparams(orc, p), None if cfg == 2 else t),
                       boundary_pairs=d["boundary_pairs"])
         assert abs(e[t].sum() - eo.sum()) <= PE_TOL * abs(eo.sum())
@@ -770,7 +776,9 @@ def test_captured_step_equals_kernel_by_kernel(monkeypatch, paper_mode):
         p = pasta.default_params(r_c=c["r_c"], thermostat_interval=10)
         if paper_mode:  # the all-pairs Coulomb kernels are captured with the rest
             p.r_nuc, p.coulomb_all_pairs = 11.5, 1
-        with pasta.Sim(8192, 0.3, 0.05, 1.0, params=p, seed=11) as sim:
+        # (the paper's mode needs a box of 120 fm: 60 000 nucleons in 126 fm, still too dense for neighbour lists)
+        size = (60000, 0.3, 0.03) if paper_mode else (8192, 0.3, 0.05)
+        with pasta.Sim(*size, 1.0, params=p, seed=11) as sim:
             sim.step(25, 2.0)
             r0 = sim.graph_replays()
             assert (r0 >= 20) if graphs == "1" else (r0 == 0)
@@ -828,6 +836,19 @@ def test_coulomb_without_cutoff_mode(orc, N, Y_P, density, path):
         assert (sim.list_stats()["list_builds"] < sim.list_stats()["force_evals"]) == (path == "list")
     with pytest.raises(pasta.PastaError):
         pasta.Sim(N, Y_P, density, 1.0, params=pasta.default_params(coulomb_all_pairs=1), seed=1)
+    # below 120 fm the mode is refused (D26): at create, and when a state, an expansion or a scaling step would go there
+    small = pasta.default_params(r_c=17.0, r_nuc=11.5, coulomb_all_pairs=1)
+    with pytest.raises(pasta.PastaError, match="120"):
+        pasta.Sim(2048, 0.4, 0.05, 1.0, params=small, seed=1)
+    shrinking = pasta.default_params(r_c=20.0, r_nuc=11.5, coulomb_all_pairs=1, scale_per_step=0.999)
+    with pasta.Sim(2000, 0.4, 2000 / 120.05 ** 3, 1.0, params=shrinking, seed=1) as sim:
+        with pytest.raises(pasta.PastaError, match="120"):
+            sim.expand(0.99)
+        with pytest.raises(pasta.PastaError, match="120"):
+            sim.step(3, 2.0)
+        xs, vs, _, Ls, _ = sim.get_state()
+        with pytest.raises(pasta.PastaError, match="120"):
+            sim.set_state(xs * 0.9, vs, None, None, 0.9 * Ls)
 
 
 @pytest.mark.parametrize("N,Y_P,density,extra", [(8192, 0.3, 0.05, {}), (20000, 0.2, 0.00125, {}),

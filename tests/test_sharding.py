@@ -78,7 +78,7 @@ def test_partition_world_size_2_gloo(tmp_path):
 @pytest.mark.gpu
 @pytest.mark.parametrize("cfg_like,world,paper_mode", [((20000, 0.3, 0.05, 17.0), 3, False), ((30000, 0.05, 0.002, 20.0), 4, False),
                                                        ((20000, 0.4, 0.01, 20.0), 3, True)])
-def test_ranks_played_in_turn_add_up_bit_exactly(cfg_like, world, paper_mode):
+def test_ranks_played_in_turn_add_up_bit_exactly(orc, cfg_like, world, paper_mode):
     """Dense chunk path, (second case: cold, dilute, wide box) the neighbour-list path, and (third) the paper's range
     split with the all-pairs Coulomb kernel, whose proton targets are sharded by the same window."""
     import torch
@@ -101,6 +101,16 @@ def test_ranks_played_in_turn_add_up_bit_exactly(cfg_like, world, paper_mode):
         # from its chunk, so that nuclear and Coulomb parts are added on one rank in the one-GPU order)
         assert int(owners.max()) == 1 and int((owners == 0).sum()) <= 2
         assert torch.equal(sum(parts), F1) and torch.equal(sum(eparts), e1)
+        # ... and the sharded evaluation against the ORACLE, at the gates of the unsharded parity tests (D17, D22)
+        from test_gpu_parity import PE_TOL, _alts, _check_forces, _np, _oparams
+
+        xs, _, is_p, L, _ = sim.get_state()
+        xs, is_p = _np(xs), _np(is_p)
+        op = orc.Params(r_c=r_c, r_nuc=11.5, coul_nocut=1.0) if paper_mode else _oparams(orc, sim.params)
+        Fo, eo, peo, d = orc.forces(xs, is_p, L, op)
+        _check_forces(_np(sum(parts)), Fo, alternates=None if paper_mode else _alts(orc, xs, is_p, L, op),
+                      boundary_pairs=d["boundary_pairs"])
+        assert abs(float(sum(eparts).sum()) - peo) <= PE_TOL * abs(peo)
         Np = int(sim.get_state()[2].sum())
         b = pasta.shard_bounds(N, Np, *sim.shard_costs(), world)
         sizes = [int((q != 0).any(dim=1).sum()) for q in parts]
@@ -122,7 +132,7 @@ torch.cuda.set_device(0)                      # both ranks share the one GPU; on
 cases = {
     "dense": (6000, 0.3, 0.05, dict(r_c=17.0, thermostat_interval=5), 12),
     "dilute_lists_scaling_box": (8000, 0.2, 0.001, dict(r_c=20.0, thermostat_interval=5, scale_per_step=1.0004), 40),
-    "paper_mode": (5000, 0.4, 0.003, dict(r_c=20.0, r_nuc=11.5, coulomb_all_pairs=1, thermostat_interval=4), 10),
+    "paper_mode": (5000, 0.4, 0.0028, dict(r_c=20.0, r_nuc=11.5, coulomb_all_pairs=1, thermostat_interval=4), 10),
 }
 out = {}
 for name, (N, Y_P, density, prm, steps) in cases.items():
