@@ -6,9 +6,12 @@ at 409 600 nucleons; fraction of the B200 FP32/SFU roofline).
 
 One "step" = one full MD step (first half kick + drift + box scaling + wrap, cell-list build, pair
 force + energy, second half kick + KE + thermostat) of BASELINE config 4 (409 600 nucleons, Y_P = 0.30,
-n = 0.08 fm^-3, T = 0.5 MeV, r_c = 20 fm, rescale every 10 steps) on seeded synthetic input.  The path
-does not shard ("replicas only"), so --gpus N runs N independent replicas, one process
-per GPU, and reports their aggregate.  Prints ONE JSON line on rank 0.
+n = 0.08 fm^-3, T = 0.5 MeV, r_c = 20 fm, rescale every 10 steps) on seeded synthetic input.  The metric
+names two sizes: the same line carries a `config2` block with the 51 200-nucleon numbers (BASELINE config 2),
+measured in the same process after the config-4 legs.  By default --gpus N runs N independent replicas, one
+process per GPU, and reports their aggregate ("replicas only"); --shard runs ONE simulation
+with the targets of every force evaluation split over the ranks instead (never measured on
+hardware: no multi-GPU node was available).  Prints ONE JSON line on rank 0.
 """
 import argparse
 import json
@@ -133,13 +136,14 @@ def cpu_baseline(cfg, budget_s, seed=1, state=None, all_pairs=True):
     p = oracle.Params(r_c=c["r_c"])
     cores = oracle.num_threads()
     t0 = time.perf_counter()
-    _, _, _, npairs = oracle.forces_cells(x, is_p, L, p)
+    _, _, pe_fp64, npairs = oracle.forces_cells(x, is_p, L, p)
     dt = time.perf_counter() - t0
     out = {
         "value": 1.0 / dt, "unit": "steps/s", "cores": cores, "kind": "oracle",
         "sample": "one full FP64 force+energy evaluation of all %d targets through the oracle's 27-cell list "
-                  "(orc_forces_cells) in %.2f s; not extrapolated" % (c["N"], dt),
-        "ordered_pairs_per_s": npairs / dt,
+                  "(orc_forces_cells) in %.2f s; not extrapolated%s" % (
+                      c["N"], dt, "; on the state read back from the GPU run after its timed steps" if state is not None else ""),
+        "ordered_pairs_per_s": npairs / dt, "PE_MeV": pe_fp64,
     }
     if all_pairs:
         rng = np.random.default_rng(0)
@@ -181,11 +185,15 @@ def run_reference(args, rank, world):
             vals.append(base["value"])
     if not vals:
         vals = [first["value"]]
+    for b_ in (first, base):  # (the state is the seeded start, not a GPU read-back)
+        b_["sample"] = b_["sample"].replace("; on the state read back from the GPU run after its timed steps", "")
     v = len(vals) / sum(1.0 / a for a in vals)
     sample = base["sample"] + "; %d evaluations timed (%d asked for, bounded to ~150 s)" % (len(vals), args.steps)
     line = {
         "impl": "reference", "metric": "md_steps_per_s", "value": v, "unit": "steps/s", "n_gpus": args.gpus,
-        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 / v, "higher_is_better": True,
+        # `steps` / `warmup` are what was really run and timed, so that steps x ms_per_step is this arm's timed region
+        "steps": len(vals), "warmup": n_run - len(vals), "steps_asked": args.steps, "warmup_asked": args.warmup,
+        "ms_per_step": 1e3 / v, "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
         "config": workload_config(args.config, world),
         "cpu_baseline": {"value": v, "unit": "steps/s", "cores": base["cores"], "kind": "oracle", "sample": sample},
@@ -221,6 +229,72 @@ def aggregate_rate(world, steps, seconds):
     return world * steps / seconds
 
 
+def device_leg(sim, c, steps, warmup, flush, barrier, clock_gpu):
+    """Device-resident timing of `steps` single MD steps, each bracketed by CUDA events on the simulation's stream (torch's
+    current one), L2 flushed in between; then the same steps once more with the library's own event brackets around the
+    kernel groups (K1 / K2 / K3) -- the brackets switch the captured-graph replay of a step off, so they are kept out of
+    the headline region.  nvidia-smi clocks are sampled over both (clock_gpu = GPU index, None = do not sample)."""
+    import torch
+
+    for _ in range(max(warmup, 3)):
+        sim.step(1, c["dt"])
+    torch.cuda.synchronize()
+    n0 = sim.launch_count()
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
+    barrier()
+    sampler = ClockSampler(clock_gpu) if clock_gpu is not None else None
+    t_wall0 = time.perf_counter()
+    for a, b in ev:
+        flush.zero_()
+        a.record()
+        sim.step(1, c["dt"])
+        b.record()
+    barrier()
+    t_wall = time.perf_counter() - t_wall0
+    launches = sim.launch_count() - n0
+    sim.set_timing(True)
+    for _ in range(min(steps, 200)):
+        flush.zero_()
+        sim.step(1, c["dt"])
+    barrier()
+    clocks = sampler.stop() if sampler else None
+    tm = sim.get_timing()
+    sim.set_timing(False)
+    per_step_ms = sorted(a.elapsed_time(b) for a, b in ev)
+    pairs, pairs_nz = sim.pair_counts()  # ordered in-range pairs; those with a term that is not exactly 0 in FP32
+    return {"wall_s": t_wall, "launches": launches, "clocks": clocks, "tm": tm, "per_step_ms": per_step_ms,
+            "dev_s": sum(per_step_ms) * 1e-3, "pairs": pairs, "pairs_nz": pairs_nz}
+
+
+def k2_roofline(c, pairs, pairs_nz, k2_s, fp32_peak):
+    """(work-performed fraction, contract-formula fraction) of the FP32 peak for one pair-kernel launch of k2_s seconds."""
+    c_fp32, _ = algorithmic_cost(c["Y_P"])
+    return ((17.0 * pairs_nz + 8.0 * c["Y_P"] ** 2 * pairs) / k2_s / fp32_peak, pairs * c_fp32 / k2_s / fp32_peak)
+
+
+def config2_block(args, flush, barrier, local_rank, fp32_peak):
+    """The 51 200-nucleon half of the metric (BASELINE config 2; Fig. 1), measured like the headline."""
+    import paper_1412_8502_b200 as pasta
+
+    c = inputs.CONFIGS[2]
+    prm = pasta.default_params(r_c=c["r_c"], thermostat_interval=c["thermostat_interval"], scale_per_step=c["scale_per_step"])
+    with pasta.Sim(c["N"], c["Y_P"], c["density"], c["T"], params=prm, seed=args.seed) as sim:
+        leg = device_leg(sim, c, args.steps, args.warmup, flush, barrier, local_rank)
+        ke, pe = sim.energy()
+    tm, n_ev = leg["tm"], max(1, leg["tm"]["force_evals"])
+    k2_s = tm["force_ms"] * 1e-3 / n_ev
+    frac, frac_contract = k2_roofline(c, leg["pairs"], leg["pairs_nz"], k2_s, fp32_peak)
+    rate = args.steps / leg["dev_s"]
+    return {"workload": workload_config(2, 1)["workload"], "N": c["N"], "md_steps_per_s": rate,
+            "ms_per_step": 1e3 * leg["dev_s"] / args.steps, "steps": args.steps,
+            "pair_interactions_per_s": {"unordered": 0.5 * leg["pairs"] * rate, "ordered": leg["pairs"] * rate,
+                                        "ordered_pairs_per_step": leg["pairs"]},
+            "kernel_ms": {"cells": tm["cells_ms"] / n_ev, "pair_force": 1e3 * k2_s, "integrate": tm["integrate_ms"] / n_ev},
+            "roofline": {"bound": "alu", "kernel": "pair force (K2)", "frac": frac, "frac_contract_formula": frac_contract,
+                         "peak": fp32_peak / 1e9, "unit": "G FP32 lane-instr/s", "nonzero_pairs_per_step": leg["pairs_nz"]},
+            "gpu_launches": leg["launches"], "clocks": leg["clocks"], "energies_MeV": {"KE": ke, "PE": pe}}
+
+
 def run_ours(args, rank, world, local_rank):
     import torch
 
@@ -254,36 +328,9 @@ def run_ours(args, rank, world, local_rank):
             dist.barrier()
         torch.cuda.synchronize()
 
-    # ---- device-resident timing: K single steps, each bracketed by events, L2 flushed in between ----
-    for _ in range(max(args.warmup, 3)):
-        sim.step(1, c["dt"])
-    torch.cuda.synchronize()
-    n0 = sim.launch_count()
-    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
-    barrier()
-    sampler = ClockSampler(local_rank) if rank == 0 else None
-    t_wall0 = time.perf_counter()
-    for a, b in ev:
-        flush.zero_()
-        a.record()
-        sim.step(1, c["dt"])
-        b.record()
-    barrier()
-    t_wall = time.perf_counter() - t_wall0
-    launches = sim.launch_count() - n0
-    # ---- the same steps once more with the library's own event brackets around the kernel groups (K1 / K2 / K3): the
-    # brackets switch the captured-graph replay of a step off, so they are kept out of the headline region above
-    sim.set_timing(True)
-    for _ in range(min(args.steps, 200)):
-        flush.zero_()
-        sim.step(1, c["dt"])
-    barrier()
-    clocks = sampler.stop() if sampler else None
-    tm = sim.get_timing()
-    sim.set_timing(False)
-    per_step_ms = sorted(a.elapsed_time(b) for a, b in ev)
-    dev_s = sum(per_step_ms) * 1e-3
-    pairs, pairs_nz = sim.pair_counts()  # ordered in-range pairs; those with a term that is not exactly 0 in FP32
+    leg = device_leg(sim, c, args.steps, args.warmup, flush, barrier, local_rank if rank == 0 else None)
+    t_wall, launches, clocks, tm, per_step_ms = leg["wall_s"], leg["launches"], leg["clocks"], leg["tm"], leg["per_step_ms"]
+    dev_s, pairs, pairs_nz = leg["dev_s"], leg["pairs"], leg["pairs_nz"]
     ke, pe = sim.energy()
 
     # ---- end to end through the C ABI with HOST buffers: every step copies the state in and out ----
@@ -383,8 +430,19 @@ def run_ours(args, rank, world, local_rank):
             "gpu_launches": launches, "wall_s": t_wall, "clocks": clocks,
             "energies_MeV": {"KE": ke, "PE": pe},
         }
+        if args.config == 4 and not args.no_config2 and world == 1:
+            line["config2"] = config2_block(args, flush, barrier, local_rank, fp32_peak)
         if not args.no_cpu_baseline and world == 1:
-            line["cpu_baseline"] = cpu_baseline(args.config, args.cpu_budget)
+            # the oracle gets the state the simulation ended in, so that its FP64 PE and the GPU's are of ONE configuration
+            xs, vs, ps, Ls, _ = sim.get_state()
+            ke_end, pe_end = sim.energy()
+            state = (xs.cpu().numpy(), vs.cpu().numpy(), ps.cpu().numpy(), Ls)
+            line["cpu_baseline"] = cpu_baseline(args.config, args.cpu_budget, state=state)
+            pe_fp64 = line["cpu_baseline"]["PE_MeV"]
+            rel = abs(pe_end - pe_fp64) / abs(pe_fp64)
+            line["pe_parity"] = {"gpu_PE_MeV": pe_end, "oracle_fp64_PE_MeV": pe_fp64, "rel": rel, "gate": 1e-6, "ok": bool(rel <= 1e-6),
+                                 "what": "total PE of all %d nucleons of the final state of this run: the CUDA path against "
+                                         "orc_forces_cells" % N}
         print(json.dumps(line), flush=True)
     sim.close()
     if dist is not None:
@@ -476,6 +534,7 @@ def main():
                     "e.g. r_nuc=11.5 (the paper's range split) or skip_exact_zeros=0")
     ap.add_argument("--cpu-budget", type=float, default=15.0, help="seconds of oracle time for cpu_baseline")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-config2", action="store_true", help="leave the 51 200-nucleon block out of the config-4 line")
     args = ap.parse_args()
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))

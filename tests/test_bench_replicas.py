@@ -62,3 +62,10 @@ def test_bench_roofline_inputs_come_from_committed_files():
     cfg = bench.workload_config(4, 1)
     assert cfg["N"] == 409600 and "workload" in cfg and "model" not in cfg
     assert "sharded" in bench.workload_config(4, 8, True)["parallelism"]
+    # the two fractions of the line and of its config2 block, on the verdict's own round-2 figures: 17 x 501 537 816
+    # non-zero pairs + 8 x 0.09 x 1 097 845 910 ordered pairs in 1.04177 ms against 148 x 128 x 1.965 GHz
+    from paper_1412_8502_b200 import inputs
+
+    peak = 148 * 128 * 1.965e9
+    frac, contract = bench.k2_roofline(inputs.CONFIGS[4], 1097845910, 501537816, 1.04177e-3, peak)
+    assert abs(frac - 0.240) < 5e-4 and abs(contract - 0.5016) < 5e-4
