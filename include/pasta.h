@@ -60,10 +60,11 @@ typedef struct pasta_params {
   int32_t skip_exact_zeros;    /* 1 (default): np/nn candidates beyond the distance at which exp2(-r^2 log2e/2 Lambda)
                                   underflows FP32 (14.78 fm for Lambda = 1.25) are not streamed: their terms are exactly
                                   0.0f in the kernel's arithmetic, so F and e are unchanged (D23).  0: stream to r_c */
-  int32_t list_reuse;          /* 1 (default): where a species is sparse the sorted order, the chunk table and every chunk's
-                                  source-segment list are built with a halo (skin) and kept across steps until some particle
-                                  has moved more than half the halo -- the paper's neighbour list with its displacement
-                                  trigger.  F and e do not depend on it.  0: rebuild every step */
+  int32_t list_reuse;          /* 1 (default): where both species are sparse the sorted order and, for EVERY TARGET, the list
+                                  of sorted source slots within reach + halo (skin) are built once and kept across steps
+                                  until some particle has moved more than half the halo -- the paper's neighbour list with
+                                  its displacement trigger.  F and e do not depend on it (to FP32
+                                  summation order).  0: rebuild the cell list every step */
   double list_halo;            /* halo thickness delta_r in fm (PAPER.md:126 uses 4 fm); 0 = library default (6 fm) */
   double r_nuc;                /* > 0: the paper's own range split: the nuclear (Gaussian) terms are zero
                                   and not computed beyond r_nuc (11.5 fm in the paper) while the Coulomb term still reaches
@@ -334,6 +335,15 @@ int pasta_shard_bounds(int64_t N, int64_t Np, double cost_p, double cost_n, int3
  * out2_host = {cost of a proton target, cost of a neutron target} for the simulation's parameters (host only). */
 int pasta_shard_costs(const pasta_sim* sim, double* out2_host);
 
+/*
+ * Environment variables read once by pasta_create.  None is needed in normal use and none changes a result beyond
+ * FP32 summation order; they exist for the tests' cross-checks and for measurements:
+ *   PASTA_FORCE_VARIANT=1  the thread-per-target pair kernel on one isotropic grid (k2_force.cu) instead of the chunk
+ *                          kernel: the in-library cross-check of the production kernel (no lists, no graphs, no stats)
+ *   PASTA_GRAPHS=0         never replay a step as a CUDA graph (see pasta_graph_replays)
+ *   PASTA_AUTO_GRID=0      both species' force grids take pasta_params.cell_subdiv instead of a k chosen per species
+ *   PASTA_X_SUBDIV=n       n thin cells per cell along x on the force grids instead of the automatic choice
+ */
 const char* pasta_last_error(void);
 const char* pasta_version(void);
 
