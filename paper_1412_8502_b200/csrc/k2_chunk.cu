@@ -36,6 +36,7 @@ namespace {
 template <bool CUT, bool ENERGY, bool STATS, int MINB>
 __global__ void __launch_bounds__(WARPS * 32, MINB) k2_chunk_kernel(const ChunkArgs A, const PairConsts c) {
   __shared__ WarpShared shared[WARPS];
+  __shared__ __align__(1024) float4 tiles[WARPS][2][32];  // a warp's double buffer: 1024 bytes, 1024-byte aligned
   const int lane = threadIdx.x & 31;
   // the warp index is produced by REDUX so that the compiler can prove it warp-uniform and keep it (and
   // everything derived from it) in uniform registers, off the vector register file
@@ -65,8 +66,9 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) k2_chunk_kernel(const ChunkA
   acc.fx = acc.fy = acc.fz = acc.e = make_float2(0.f, 0.f);
   unsigned long long st[3] = {0, 0, 0};
 
-  chunk_passes<CUT, ENERGY, STATS, MINB == K2_MINB_SPARSE>(A, c, sh, lane, pr, gt, st_sp, chunk_p, tp, tc, active, acc,
-                                                           st);
+  const unsigned tile_a = (unsigned)__cvta_generic_to_shared(&tiles[wib][0][0]);
+  chunk_passes<CUT, ENERGY, STATS, MINB == K2_MINB_SPARSE>(A, c, sh, tile_a, lane, pr, gt, st_sp, chunk_p, tp, tc, active,
+                                                           acc, st);
 
   write_chunk_results<ENERGY>(A, c, acc, lane, slot);
   if (STATS && lane == 0) {

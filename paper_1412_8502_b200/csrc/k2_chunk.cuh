@@ -76,9 +76,10 @@ struct ChunkArgs {
 //             xoff: add to pos4.w (thin-cell index) to get the cell offset from the frame's reference
 //             cell; yoff, zoff: the row's offsets from the reference cell centre, times the cell width
 //   cum[k]  = stream position at which segment k starts (cum[nseg] = stream length, then +infinity)
-//   tile    = the sources of two consecutive tiles in the chunk's frame (double buffer)
+// The tiles themselves -- the sources of two consecutive tiles in the chunk's frame, a double buffer of 2 x 512 bytes per
+// warp -- live in an array of their own (k2_chunk_kernel), 1024-byte aligned, so that the two buffers of a warp differ
+// in exactly one address bit and the toggle is a single XOR.
 struct WarpShared {
-  float4 tile[2][32];
   float4 seg[SEG_CAP + 1];
   int cum[SEG_CAP + 1 + 32];
   float flag[SEG_CAP + 1];  // BOTH-species streams: 0 = the segment holds protons, 1 = neutrons
@@ -195,8 +196,8 @@ __device__ __forceinline__ float4 to_frame(const float4 q, const float4 m, const
 // STEPS sources of the tile against its pair of targets.  Positions past the end of the stream become idle
 // sources ~1e11 away, which contribute exact zeros.
 template <bool COUL, bool CUT, bool ENERGY, bool STATS, bool BOTH>
-__device__ __forceinline__ void run_stream(const ChunkArgs& A, const PairConsts& c, WarpShared& sh, const int lane,
-                                           const int total, const float wxS, const Targets& t, Accum& acc,
+__device__ __forceinline__ void run_stream(const ChunkArgs& A, const PairConsts& c, WarpShared& sh, const unsigned tile_a,
+                                           const int lane, const int total, const float wxS, const Targets& t, Accum& acc,
                                            const PassConsts& k, unsigned long long* st) {
   if (total == 0) return;
   const int ntile = (total + 31) >> 5;
@@ -208,11 +209,10 @@ __device__ __forceinline__ void run_stream(const ChunkArgs& A, const PairConsts&
   cu.flag = BOTH ? sh.flag[0] : 0.f;
   float4 q, m;
   fetch<BOTH>(A, sh, cu, lane, total, q, m);
-  // shared-window addresses of this lane's store slot and first load slot; the double buffer is toggled by reflecting
-  // the address about the middle of the two buffers (one integer instruction each)
-  unsigned wr_a = (unsigned)__cvta_generic_to_shared(&sh.tile[0][lane]);
-  unsigned rd_a = (unsigned)__cvta_generic_to_shared(&sh.tile[0][ph]);
-  const unsigned wr_c = 2u * wr_a + 512u, rd_c = 2u * rd_a + 512u;
+  // shared-window addresses of this lane's store slot and first load slot in buffer 0 (tile_a is 1024-byte aligned, the
+  // second buffer sits 512 bytes above the first: the toggle flips address bit 9)
+  unsigned wr_a = tile_a + 16u * (unsigned)lane;
+  unsigned rd_a = tile_a + 16u * (unsigned)ph;
 #pragma unroll 1
   for (int i = 0; i < ntile; ++i) {
     const float4 s = to_frame<BOTH>(q, m, wxS);
@@ -225,8 +225,8 @@ __device__ __forceinline__ void run_stream(const ChunkArgs& A, const PairConsts&
     evaluate<COUL, CUT, ENERGY, BOTH>(lds128<NPH * 16>(rd_a), t, acc, k, c);
     evaluate<COUL, CUT, ENERGY, BOTH>(lds128<NPH * 32>(rd_a), t, acc, k, c);
     evaluate<COUL, CUT, ENERGY, BOTH>(lds128<NPH * 48>(rd_a), t, acc, k, c);
-    wr_a = wr_c - wr_a;
-    rd_a = rd_c - rd_a;
+    wr_a ^= 512u;
+    rd_a ^= 512u;
   }
   __syncwarp();
   if (STATS && lane == 0) {
@@ -246,8 +246,8 @@ struct Box {
 // BOTH: the two species share one grid geometry (gs = either) and the pass lists the segments of both, every row
 // once: a "round" is then a (periodic image, species) pair.
 template <bool COUL, bool CUT, bool ENERGY, bool STATS, bool BOTH>
-__device__ __forceinline__ void source_pass(const ChunkArgs& A, const PairConsts& c, WarpShared& sh, const int lane,
-                                            const SpeciesGrid& gs, const int rx, const int ry, const int rz,
+__device__ __forceinline__ void source_pass(const ChunkArgs& A, const PairConsts& c, WarpShared& sh, const unsigned tile_a,
+                                            const int lane, const SpeciesGrid& gs, const int rx, const int ry, const int rz,
                                             const Box& b, const Targets& t, Accum& acc, const PassConsts& k,
                                             unsigned long long* st) {
   const float half = 0.5f * gs.wS;
@@ -336,7 +336,7 @@ __device__ __forceinline__ void source_pass(const ChunkArgs& A, const PairConsts
     sh.cum[nseg_list + lane] = lane == 0 ? total : 0x3fffffff;
     if (lane == 0) sh.cum[nseg_list + 32] = 0x3fffffff;
     __syncwarp();
-    run_stream<COUL, CUT, ENERGY, STATS, BOTH>(A, c, sh, lane, total, gs.wxS, t, acc, k, st);
+    run_stream<COUL, CUT, ENERGY, STATS, BOTH>(A, c, sh, tile_a, lane, total, gs.wxS, t, acc, k, st);
   } while (rbase < nrows);
 }
 
@@ -354,8 +354,8 @@ __device__ __forceinline__ int min_image_cells(int m, int nc) {
 // MERGE: on identical grids a neutron chunk takes both source species in ONE pass (one listing instead of two: it
 // is the listing, not the arithmetic, that a sparse system pays for).
 template <bool CUT, bool ENERGY, bool STATS, bool MERGE>
-__device__ __forceinline__ void chunk_passes(const ChunkArgs& A, const PairConsts& c, WarpShared& sh, const int lane,
-                                             const int pr, const SpeciesGrid& gt, const int st_sp, const bool chunk_p,
+__device__ __forceinline__ void chunk_passes(const ChunkArgs& A, const PairConsts& c, WarpShared& sh, const unsigned tile_a,
+                                             const int lane, const int pr, const SpeciesGrid& gt, const int st_sp, const bool chunk_p,
                                              const float4 tp, const int tc, const unsigned active, Accum& acc,
                                              unsigned long long* st) {
   const bool mine = ((active >> lane) & 1u) != 0;
@@ -440,14 +440,17 @@ __device__ __forceinline__ void chunk_passes(const ChunkArgs& A, const PairConst
     k.B = like ? c.B_like : c.B_unlike;
     k.gB_n = c.gB_like;  // (BOTH: neutron targets; proton sources are unlike, neutron sources like)
     k.B_n = c.B_like;
+    // the selected isospin constants stay in registers: without this the tile loop of the unlike-species pass re-derives
+    // them from the constant bank every iteration (a compare, two loads, two predicated loads: 5 of its 108 instructions)
+    asm volatile("" : "+f"(k.gB), "+f"(k.B));
     if (MERGE && both) {
       k.gB = c.gB_unlike;
       k.B = c.B_unlike;
-      source_pass<false, CUT, ENERGY, STATS, true>(A, c, sh, lane, gs, rx, ry, rz, b, t, acc, k, st);
+      source_pass<false, CUT, ENERGY, STATS, true>(A, c, sh, tile_a, lane, gs, rx, ry, rz, b, t, acc, k, st);
     } else if (sp == 0 && chunk_p && A.no_coul == 0) {
-      source_pass<true, CUT, ENERGY, STATS, false>(A, c, sh, lane, gs, rx, ry, rz, b, t, acc, k, st);
+      source_pass<true, CUT, ENERGY, STATS, false>(A, c, sh, tile_a, lane, gs, rx, ry, rz, b, t, acc, k, st);
     } else {
-      source_pass<false, CUT, ENERGY, STATS, false>(A, c, sh, lane, gs, rx, ry, rz, b, t, acc, k, st);
+      source_pass<false, CUT, ENERGY, STATS, false>(A, c, sh, tile_a, lane, gs, rx, ry, rz, b, t, acc, k, st);
     }
   }
 }
