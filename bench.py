@@ -51,7 +51,7 @@ def ncu_traffic(cfg):
     import re
 
     unit = {"byte": 1.0, "Kbyte": 1e3, "Mbyte": 1e6, "Gbyte": 1e9}
-    for name in ("r2_k2_ncu_cfg%d.md" % cfg,):
+    for name in ("r3_k2_ncu_cfg%d.md" % cfg, "r2_k2_ncu_cfg%d.md" % cfg):  # the newest capture of the shipped kernel first
         path = os.path.join(ROOT, "profiles", name)
         if not os.path.exists(path):
             continue
