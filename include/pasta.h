@@ -316,8 +316,9 @@ int64_t pasta_graph_replays(const pasta_sim* sim);
  * decomposition with Q = 1).  Every rank holds the WHOLE state (positions, velocities, species) and keeps it
  * bit-identical; of every force evaluation it computes only the targets of its own stretch of the cell-sorted order
  * (the sorted slots [bounds[rank], bounds[rank+1]) of pasta_shard_bounds: contiguous in space along the sort, balanced
- * by the estimated pair work of the two species), leaves zeros elsewhere, and the ranks' partial F (3 N doubles) and e
- * (N doubles) are then summed in place by `allreduce` -- the paper's MPI_Allreduce of the forces; every
+ * by the estimated pair work of the two species), leaves zeros elsewhere, and the ranks' partial F and e -- stored back
+ * to back, so ONE call on 4 N doubles, or on the 3 N of F alone when an evaluation computes no energies -- are then
+ * summed in place by `allreduce`: the paper's MPI_Allreduce of the forces; every
  * particle's force is complete on exactly one rank, so the sum is exact and the result is bit-identical to the
  * one-GPU evaluation.  Cell list and integration are replicated (they cost a few % of a step).
  *   allreduce(dev_ptr, n, user): sum the n doubles at dev_ptr over all ranks, in place, ordered with the simulation's

@@ -59,7 +59,8 @@ void buffer_release(Sim* s, Buffer* b) {
 }
 
 static void release_all(Sim* s) {
-  Buffer* bs[] = {&s->x, &s->v, &s->F, &s->e, &s->is_p, &s->cell_id, &s->bin_count, &s->bin_start, &s->scan_tmp,
+  s->e = Buffer();  // an alias into s->F's allocation (pasta_create), nothing of its own to free
+  Buffer* bs[] = {&s->x, &s->v, &s->F, &s->is_p, &s->cell_id, &s->bin_count, &s->bin_start, &s->scan_tmp,
                   &s->perm, &s->perm_raw, &s->pos4, &s->cxyz, &s->cpos, &s->partials, &s->scalars, &s->counters, &s->cl_parent, &s->cl_A,
                   &s->cl_Z, &s->cl_cell_id, &s->cl_count, &s->cl_start, &s->cl_perm, &s->chunk_tab, &s->chunk_first, &s->xref, &s->slot_of, &s->list_off,
                   &s->list_pool};
@@ -137,16 +138,15 @@ static int evaluate_forces_tail(Sim* s, bool with_energy, double kick = 0.0) {
   PASTA_TRY(shard_window(s));
   {
     Timer t(s, 1);
-    if (sharded) {  // the other ranks' targets stay zero: the sum over ranks then completes every particle exactly
-      PASTA_CUDA_OK(cudaMemsetAsync(s->F.ptr, 0, 24 * (size_t)s->N, s->stream));
-      if (with_energy) PASTA_CUDA_OK(cudaMemsetAsync(s->e.ptr, 0, 8 * (size_t)s->N, s->stream));
-    }
+    // the other ranks' targets stay zero: the sum over ranks then completes every particle exactly.  F and e are one
+    // contiguous run ([F | e], pasta_create): one memset and one collective cover both
+    const size_t shard_doubles = (with_energy ? 4 : 3) * (size_t)s->N;
+    if (sharded) PASTA_CUDA_OK(cudaMemsetAsync(s->F.ptr, 0, 8 * shard_doubles, s->stream));
     if (s->list.valid) PASTA_TRY(k2_list_forces(s, with_energy));
     else PASTA_TRY(k2_forces(s, with_energy, kick));
     if (s->prm.coulomb_all_pairs) PASTA_TRY(k2_coulomb_all_pairs(s, with_energy));
     if (sharded) {
-      if (s->shard.allreduce(s->F.ptr, 3 * s->N, s->shard.user) != 0 ||
-          (with_energy && s->shard.allreduce(s->e.ptr, s->N, s->shard.user) != 0)) {
+      if (s->shard.allreduce(s->F.ptr, (int64_t)shard_doubles, s->shard.user) != 0) {
         set_error("pasta_set_shard: the allreduce callback failed");
         return PASTA_ECUDA;
       }
@@ -520,12 +520,16 @@ int pasta_create(pasta_sim** out, int64_t N, double Y_P, double density, double 
     if ((rc = use_device(s)) != PASTA_OK) break;
     const size_t n = (size_t)N;
     if ((rc = buffer_reserve(s, &s->x, 24 * n)) || (rc = buffer_reserve(s, &s->v, 24 * n)) ||
-        (rc = buffer_reserve(s, &s->F, 24 * n)) || (rc = buffer_reserve(s, &s->e, 8 * n)) ||
+        (rc = buffer_reserve(s, &s->F, 32 * n)) ||  // [F | e]: one allocation, see below
         (rc = buffer_reserve(s, &s->is_p, n)) || (rc = buffer_reserve(s, &s->cell_id, 4 * n)) ||
         (rc = buffer_reserve(s, &s->perm, 4 * n)) || (rc = buffer_reserve(s, &s->pos4, 16 * n + 4096)) ||
         (rc = buffer_reserve(s, &s->cxyz, 4 * n)) || (rc = buffer_reserve(s, &s->partials, 8 * 8192)) ||
         (rc = buffer_reserve(s, &s->scalars, 8 * 16)) || (rc = buffer_reserve(s, &s->counters, 8 * 32)))
       break;
+    // e sits right behind F (N is fixed for the life of the simulation), so that a sharded evaluation zeroes and sums
+    // forces and energies as ONE contiguous run of 4 N doubles: one memset, one collective (pasta_set_shard)
+    s->e.ptr = s->F.as<char>() + 24 * n;
+    s->e.bytes = 8 * n;
     {
       void* mb = nullptr;
       if (cudaHostAlloc(&mb, 64, cudaHostAllocMapped) != cudaSuccess ||

@@ -95,7 +95,7 @@ def test_ranks_played_in_turn_add_up_bit_exactly(orc, cfg_like, world, paper_mod
             F, _ = sim.forces()
             parts.append(F.clone())
             eparts.append(sim.particle_energies().clone())
-        assert calls == [3 * N, N] * world
+        assert calls == [4 * N] * world   # forces and energies are summed as one contiguous run: one collective per evaluation
         owners = sum((q != 0).any(dim=1).to(torch.int32) for q in parts)
         # every particle on exactly one rank (in the paper's mode too: the all-pairs Coulomb kernel takes a proton's owner
         # from its chunk, so that nuclear and Coulomb parts are added on one rank in the one-GPU order)
